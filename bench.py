@@ -1,0 +1,343 @@
+#!/usr/bin/env python
+"""bench.py -- pair-interactions/s of the direct-summation hot path on B200 (BASELINE.json `metric`).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 2] [--n N]
+
+One STEP = one pass of the whole hot path over one batch of synthetic input:
+    pp_step_kdk(1 step, PP_ACC_VALID, pot)  = kick+drift+pack -> pair sweep with potential -> split-j finalize + kick
+    pp_invariants(pot)                      = E, P, L, COM, M from the state and that potential
+i.e. N(N-1) ordered pair interactions per step.  The workload is BASELINE.json configs[2] (N = 2^20 exponential
+disk, delta = 0.005, dt = 2.5e-4, seed 2) -- the configuration the metric is quoted on.  `value` is the FP32 figure
+(dtype "f32"); the same step in FP64 is timed in the same run and reported under "fp64", and the force-only single
+evaluation (pp_forces without potential) of both precisions under "force_only".
+
+Multi-GPU: the north_star runs on one GPU with no sharding -- `--gpus N` runs N independent replicas ("replicas
+only"), one process per GPU under torchrun, no data-path collective; value = pairs of all ranks / max time.
+
+--impl reference times the CPU oracle (oracle/, as it stands) on the host cores on a bounded sample of the same
+workload; it is the only other place besides cpu_baseline where this file touches oracle/.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "pair-interactions/s"
+UNIT = "pair-interactions/s"
+# nominal pipe peaks: lanes per SM x SMs x max SM clock
+FP32_LANES, FP64_LANES, SM_COUNT, SM_MAX_HZ = 128, 64, 148, 1.965e9
+L2_FLUSH_BYTES = 256 << 20
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="index into BASELINE.json configs (default 2: N=2^20)")
+    ap.add_argument("--n", type=int, default=None, help="override N (same recipe and seed)")
+    ap.add_argument("--no-fp64", action="store_true", help="skip the FP64 arm (faster profiling runs)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def workload_name(c):
+    return "configs[%d] %s N=%d delta=%g dt=%g seed=%d" % (c["index"], c["name"], c["N"], c["delta"], c["dt"],
+                                                            c["seed"])
+
+
+# ---- clocks ------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        mhz, mx, pw, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for line in self.f:
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                mhz.append(float(parts[0]))
+                mx.append(float(parts[1]))
+                pw.append(float(parts[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        self.f.close()
+        os.unlink(self.f.name)
+        if mhz:
+            out.update(sm_mhz=float(np.median(mhz)), sm_max_mhz=float(max(mx)), reasons=sorted(reasons),
+                       samples=len(mhz), power_w_max=float(max(pw)))
+        return out
+
+
+# ---- our arm -----------------------------------------------------------------------------------------------------
+def time_steps(torch, step_fn, steps, warmup, flush, barrier):
+    """W warm-up steps, then exactly K steps between two (barrier + synchronize) brackets, timed with CUDA events on
+    the current stream (the stream the library launches on).  Returns milliseconds for the K steps."""
+    for _ in range(warmup):
+        step_fn()
+        flush()
+    barrier()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        step_fn()
+        flush()
+    e1.record()
+    torch.cuda.synchronize()
+    barrier()
+    return e0.elapsed_time(e1)
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1803_01190_b200 import ppgrav, workloads
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+
+    def max_over_ranks(x):
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)      # timing bookkeeping only: not on the data path
+        return float(t.item())
+
+    ppgrav.lib()                                       # fails loudly if the CUDA library is missing
+    c = workloads.config(args.config, N=args.n)
+    c["index"] = args.config
+    if world > 1:                                      # replicas: same recipe, a different seed per rank
+        c = dict(c)
+        c["seed"] = c["seed"] + 1000 * rank
+        c["pos"], c["vel"], c["mass"] = workloads.make(c["kind"], c["N"], c["seed"], c.get("sigma_f", 0.1), c["G"])
+    N, G, delta = c["N"], c["G"], c["delta"]
+    dt = c["dt"] if c["dt"] > 0 else 2.5e-4
+    pairs = float(N) * float(N - 1)
+    flush_buf = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device="cuda")
+
+    def flush():
+        flush_buf.zero_()                              # > 126 MB L2: the next step starts cold
+
+    results = {}
+    clocks = None
+    launches = None
+    precisions = [("f32", torch.float32)] + ([] if args.no_fp64 else [("f64", torch.float64)])
+    for name, dtype in precisions:
+        pos = torch.tensor(c["pos"], dtype=dtype, device="cuda")
+        vel = torch.tensor(c["vel"], dtype=dtype, device="cuda")
+        mass = torch.tensor(c["mass"], dtype=dtype, device="cuda")
+        acc = torch.empty_like(pos)
+        pot = torch.empty_like(mass)
+        out16 = torch.empty(16, dtype=torch.float64, device="cuda")
+        ppgrav.pp_step_kdk(pos, vel, mass, acc, dt, 0, G=G, delta=delta)          # a(t0), untimed
+
+        def step():
+            ppgrav.pp_step_kdk(pos, vel, mass, acc, dt, 1, G=G, delta=delta, acc_valid=True, pot=pot)
+            ppgrav.pp_invariants(pos, vel, mass, G=G, delta=delta, pot=pot, out16=out16)
+
+        ppgrav.pp_configure(ppgrav.PP_CFG_PROFILE, 1)
+        sampler = ClockSampler(local) if (name == "f32" and rank == 0) else None
+        n0 = ppgrav.pp_launch_count()
+        # warm-up happens inside time_steps; its sweeps are discarded from the profile below
+        for _ in range(args.warmup):
+            step()
+            flush()
+        ppgrav.pp_profile_read()
+        n0 = ppgrav.pp_launch_count()
+        ms = time_steps(torch, step, args.steps, 0, flush, barrier)
+        n1 = ppgrav.pp_launch_count()
+        sweep_ms, sweep_n = ppgrav.pp_profile_read()
+        ppgrav.pp_configure(ppgrav.PP_CFG_PROFILE, 0)
+        if sampler is not None:
+            clocks = sampler.stop()
+            launches = n1 - n0
+        ms = max_over_ranks(ms)
+        plan = ppgrav.pp_plan_query(N, ppgrav.PP_F32 if name == "f32" else ppgrav.PP_F64, True)
+        lanes = FP32_LANES if name == "f32" else FP64_LANES
+        peak = lanes * SM_COUNT * SM_MAX_HZ / 1e12
+        ops = plan["pipe_ops_per_pair"]
+        achieved = ops * pairs * sweep_n / (sweep_ms * 1e-3) / 1e12 if sweep_ms > 0 else 0.0
+        inv = ppgrav.invariants_dict(out16)
+        results[name] = dict(
+            value=world * pairs * args.steps / (ms * 1e-3), ms_per_step=ms / args.steps,
+            sweep_ms_per_launch=sweep_ms / max(sweep_n, 1), sweep_share_of_step=sweep_ms / ms,
+            roofline=dict(bound="alu", kernel="force_%s_kernel (pair sweep with potential)" % name,
+                          achieved=achieved, peak=peak, unit="Tlane-op/s", frac=achieved / peak, traffic=None,
+                          pipe_ops_per_pair=ops,
+                          peak_source="nominal: %d %s lanes/SM x %d SMs x %.0f MHz" %
+                                      (lanes, "FP32" if name == "f32" else "FP64", SM_COUNT, SM_MAX_HZ / 1e6)),
+            plan=plan, E_after=inv["E"])
+
+        # force-only single evaluation (12 / 16 pipe operations per pair)
+        def force_only():
+            ppgrav.pp_forces(pos, mass, G=G, delta=delta, acc=acc)
+
+        fms = max_over_ranks(time_steps(torch, force_only, max(2, args.steps // 2), 1, flush, barrier))
+        results[name]["force_only"] = world * pairs * max(2, args.steps // 2) / (fms * 1e-3)
+
+        if name == "f32" and not args.no_e2e:
+            # end to end through the host-buffer C ABI: pinned host arrays in, results back, every step
+            hp, hv, hm, ha, hpot = (torch.empty(s, dtype=dtype).pin_memory().numpy()
+                                    for s in ((N, 3), (N, 3), (N,), (N, 3), (N,)))
+            hp[...], hv[...], hm[...] = c["pos"], c["vel"], c["mass"]
+            ha[...] = acc.cpu().numpy()
+            el = dtype.itemsize if hasattr(dtype, "itemsize") else 4
+
+            def e2e_step():
+                ppgrav.pp_step_kdk_host(hp, hv, hm, ha, dt, 1, G=G, delta=delta, acc_valid=True, pot=hpot)
+                ppgrav.pp_invariants_host(hp, hv, hm, G=G, delta=delta, pot=hpot)
+
+            for _ in range(max(1, args.warmup // 2)):
+                e2e_step()
+            barrier()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            for _ in range(args.steps):
+                e2e_step()
+                flush()
+            torch.cuda.synchronize()
+            ems = max_over_ranks((time.perf_counter() - t0) * 1e3)
+            results[name]["e2e"] = dict(value=world * pairs * args.steps / (ems * 1e-3), unit=UNIT,
+                                        h2d_bytes_per_step=int((10 * N + 8 * N) * el),
+                                        d2h_bytes_per_step=int((10 * N) * el + 128),
+                                        api="pp_step_kdk_host + pp_invariants_host (pinned host buffers)")
+        del pos, vel, mass, acc, pot
+
+    line = None
+    if rank == 0:
+        r32 = results["f32"]
+        line = {
+            "metric": METRIC, "value": r32["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": r32["ms_per_step"], "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": workload_name(c), "step": "pp_step_kdk(1 step, with potential) + pp_invariants",
+                       "pairs_per_step": pairs, "l2": "256 MiB flush write between steps, inside the timed region",
+                       "parallelism": "replicas only" if world > 1 else "single GPU"},
+            "roofline": r32["roofline"],
+            "e2e": r32.get("e2e"),
+            "gpu_launches": launches,
+            "clocks": clocks,
+            "sweep_ms_per_launch": r32["sweep_ms_per_launch"], "sweep_share_of_step": r32["sweep_share_of_step"],
+            "force_only": {k: results[k]["force_only"] for k in results},
+            "plan": r32["plan"],
+        }
+        if "f64" in results:
+            r64 = results["f64"]
+            line["fp64"] = {"value": r64["value"], "unit": UNIT, "ms_per_step": r64["ms_per_step"],
+                            "roofline": r64["roofline"], "sweep_ms_per_launch": r64["sweep_ms_per_launch"],
+                            "plan": r64["plan"], "fp64_over_fp32_time": r64["ms_per_step"] / r32["ms_per_step"]}
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(c, n_sample=16384)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return line
+
+
+# ---- the oracle on the host cores --------------------------------------------------------------------------------
+def cpu_baseline(c, n_sample):
+    """Times oracle.forces (as it stands) on a bounded sample of i-bodies against all N j-bodies."""
+    from oracle import oracle
+    from paper_1803_01190_b200 import workloads
+    idx = workloads.sample_indices(c["seed"], c["N"], n_sample)
+    cores = oracle.max_threads()
+    t0 = time.perf_counter()
+    oracle.forces(c["pos"], c["mass"], G=c["G"], delta=c["delta"], idx=idx, want_pot=True, nthreads=0)
+    sec = time.perf_counter() - t0
+    pairs = float(len(idx)) * float(c["N"] - 1)
+    return {"value": pairs / sec, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": sec,
+            "sample": "oracle.forces (FP64, compensated sums, OpenMP over i) for %d sampled i-bodies x all %d "
+                      "j-bodies of the same workload = %.3g pairs" % (len(idx), c["N"], pairs)}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return None
+    from oracle import oracle
+    from paper_1803_01190_b200 import workloads
+    oracle.build()
+    c = workloads.config(args.config, N=args.n)
+    c["index"] = args.config
+    n_sample = 4096                                   # per step: 4096 i-bodies x N j-bodies (4.3e9 pairs at N=2^20)
+    idx = workloads.sample_indices(c["seed"], c["N"], n_sample)
+    cores = oracle.max_threads()
+    pairs = float(len(idx)) * float(c["N"] - 1)
+
+    def step():
+        oracle.forces(c["pos"], c["mass"], G=c["G"], delta=c["delta"], idx=idx, want_pot=True, nthreads=0)
+
+    for _ in range(args.warmup):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    sec = time.perf_counter() - t0
+    value = pairs * args.steps / sec
+    sample = ("each step = oracle.forces (FP64, compensated sums, OpenMP over i) for %d sampled i-bodies x all %d "
+              "j-bodies = %.3g pairs" % (len(idx), c["N"], pairs))
+    return {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec * 1e3 / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(c), "step": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+
+
+def main():
+    args = parse_args()
+    line = run_reference(args) if args.impl == "reference" else run_ours(args)
+    if line is not None:
+        print(json.dumps(line), flush=True)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,129 @@
+/* ppgrav.h -- C ABI of libppgrav: direct particle-particle (PP) gravity on one NVIDIA B200 (sm_100a).
+ *
+ * The library implements the hot path of Khrapov, Khoperskov & Khoperskov, "New features of parallel
+ * implementation of N-body problems on GPU" (2018); citations are PAPER.md:<line> of /root/reference/PAPER.md.
+ *
+ *   pp_forces      eq. (1)-(2), PAPER.md:41-48   a_i = -G sum_{j != i} m_j (r_i - r_j) / (|r_i - r_j|^2 + delta^2)^{3/2}
+ *                                                Phi_i = -G sum_{j != i} m_j / (|r_i - r_j|^2 + delta^2)^{1/2}
+ *   pp_step_kdk    eqs. (5)-(7), PAPER.md:67-92  kick-drift-kick leapfrog, one gravity solve per step
+ *   pp_invariants  eqs. (8)-(10), PAPER.md:148-156  E = K + W, P, L, centre of mass, total mass
+ *
+ * Conventions common to every call
+ *   - Plain C, no exceptions.  Every function returns an int status: PP_OK (0) or a negative PP_E* code;
+ *     pp_last_error() then returns a human-readable message for the calling thread.
+ *   - Unless the name ends in _host, every data pointer is a DEVICE pointer on the current CUDA device, owned by
+ *     the caller; the library never frees or retains it.  Work is enqueued on `stream` (a cudaStream_t passed as
+ *     void*; NULL = the legacy default stream) and the call returns without synchronising.
+ *   - _host variants take HOST pointers (pageable or pinned), copy in, run the same kernels, copy out and
+ *     synchronise `stream` before returning.
+ *   - Layout: pos, vel, acc are row-major [N,3]; mass, pot are [N]; element type float (PP_F32) or double
+ *     (PP_F64) according to `precision`; pointers must be aligned to the element size.  No padding is required.
+ *   - delta is the Plummer softening length of PAPER.md:48 (delta >= 0).  delta == 0 is legal: pairs at zero
+ *     distance (including padding and j == i) then contribute nothing.
+ *   - G multiplies the finished sums once (acc = G * sum), not every pair.
+ *   - Results are bit-reproducible run to run for the same N, plan and device (no floating-point atomics).
+ *   - The library keeps a per-device workspace (packed copy of the bodies, split-j partial sums) that grows on
+ *     demand and is freed by pp_release().  Calls that share a device must therefore be issued on one stream at a
+ *     time (stream-ordered reuse); concurrent use from several streams is not supported.
+ *   - There is no CPU fallback: without a CUDA device every compute call returns PP_ECUDA.
+ */
+#ifndef PPGRAV_H_
+#define PPGRAV_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PPGRAV_VERSION 100 /* 0.1.0 */
+
+/* precision */
+#define PP_F32 0
+#define PP_F64 1
+
+/* status codes */
+#define PP_OK 0
+#define PP_EINVAL (-1) /* NULL / misaligned pointer, N < 1, delta < 0, non-finite scalar, bad precision/flags */
+#define PP_ECUDA (-2)  /* a CUDA runtime call failed (message in pp_last_error) */
+#define PP_ENOMEM (-3) /* workspace allocation failed */
+
+/* pp_step_kdk flags */
+#define PP_ACC_VALID 1u /* acc already holds a(t0) for the incoming positions: skip the initial gravity solve */
+
+/* pp_configure keys */
+#define PP_CFG_SPLIT_J 1 /* 0 = automatic (default); S >= 1 forces the j-range to be split S ways */
+#define PP_CFG_GRAPH 2   /* 1 (default) = pp_step_kdk replays its step loop from a CUDA graph when N is small */
+#define PP_CFG_PROFILE 3 /* 1 = bracket every pair-sweep launch with CUDA events (pp_profile_read); no graph replay */
+
+/* Version of the library that was loaded (PPGRAV_VERSION). */
+int pp_version(void);
+
+/* Message of the last error raised on the calling thread ("" if none). */
+const char* pp_last_error(void);
+
+/* Free the cached workspace of `device` (-1: all devices).  Synchronises that device. */
+int pp_release(int device);
+
+/* Tuning / test hook, see PP_CFG_*.  Process-wide. */
+int pp_configure(int key, int64_t value);
+
+/* Number of CUDA kernels this library has launched since it was loaded (all threads). */
+int64_t pp_launch_count(void);
+
+/* With PP_CFG_PROFILE on: waits for the recorded pair-sweep launches and returns out2 (host) =
+ * { their summed device time in milliseconds, their number } since the previous read, then forgets them.
+ * This is how bench.py obtains the average duration of the dominant kernel without a profiler. */
+int pp_profile_read(double* out2);
+
+/* Gravity solve, eq. (1)-(2): the paper's "Gravity Force Computation" kernel.
+ *   pos  [N,3] in,  mass [N] in,  acc [N,3] out,  pot [N] out or NULL (skip the potential).
+ * O(N^2): N(N-1) ordered pair interactions.  PP_F32: FP32 pair arithmetic, FP32 blocked + compensated sums.
+ * PP_F64: FP64 throughout.  acc/pot must not alias pos/mass. */
+int pp_forces(const void* pos, const void* mass, void* acc, void* pot, int64_t N, double G, double delta,
+              int precision, void* stream);
+
+/* nsteps kick-drift-kick steps of size dt, eqs. (5)-(7), in the algebraically identical
+ * half-kick form  v += dt/2 a(t);  r += dt v;  a(t+dt) = forces(r);  v += dt/2 a(t+dt)  -- the paper's "Update
+ * System" kernel around one gravity solve per step.
+ *   pos, vel [N,3] in/out;  mass [N] in;  acc [N,3] in/out: with PP_ACC_VALID it holds a(t0) on entry (no initial
+ *   solve); on return it always holds a(t0 + nsteps*dt), ready to be passed back with PP_ACC_VALID.
+ *   pot [N] out or NULL: if given, the LAST gravity solve of the call also produces Phi_i at t0 + nsteps*dt in the
+ *   state precision (one more pipe operation per pair in that solve only), ready for pp_invariants; if the call
+ *   performs no solve (nsteps == 0 with PP_ACC_VALID) pot is left untouched.
+ * nsteps == 0 only (re)computes acc.  Force evaluations performed: nsteps (+1 without PP_ACC_VALID). */
+int pp_step_kdk(void* pos, void* vel, const void* mass, void* acc, void* pot, int64_t N, double dt, int64_t nsteps,
+                double G, double delta, int precision, unsigned flags, void* stream);
+
+/* Conserved integrals, eqs. (8)-(10) plus centre of mass (Fig. 6).
+ *   out16 (device, 16 doubles) = { E, K, W, Px, Py, Pz, Lx, Ly, Lz, Cx, Cy, Cz, M, 0, 0, 0 }
+ *   K = sum m v^2/2;  W = (1/2) sum_i m_i Phi_i  (negative; j != i);  E = K + W;  P = sum m v;  L = sum m r x v.
+ * State arrays are `precision`; all sums are accumulated in FP64 with compensation regardless.
+ *   pot: Phi_i [N] in the state precision as returned by pp_forces, or NULL -- then an O(N^2) FP64 potential pass
+ *   with compensated accumulation is run on the (promoted) state. */
+int pp_invariants(const void* pos, const void* vel, const void* mass, const void* pot, int64_t N, double G,
+                  double delta, int precision, double* out16, void* stream);
+
+/* Host-buffer variants: same semantics, HOST pointers, synchronous (copies in, computes, copies out). */
+int pp_forces_host(const void* pos, const void* mass, void* acc, void* pot, int64_t N, double G, double delta,
+                   int precision, void* stream);
+int pp_step_kdk_host(void* pos, void* vel, const void* mass, void* acc, void* pot, int64_t N, double dt,
+                     int64_t nsteps, double G, double delta, int precision, unsigned flags, void* stream);
+int pp_invariants_host(const void* pos, const void* vel, const void* mass, const void* pot, int64_t N, double G,
+                       double delta, int precision, double* out16, void* stream);
+
+/* Launch plan the library would use for a gravity solve of N bodies: out8 (host) =
+ *   { i-bodies per CTA, j-bodies per tile, split-j factor S, CTAs launched, CTAs resident per SM, SM count,
+ *     pipe operations per pair (FP32- or FP64-pipe instructions per lane), MUFU operations per pair }. */
+int pp_plan_query(int64_t N, int precision, int with_pot, int64_t* out8);
+
+/* Pipe-throughput microbenchmark used for the roofline denominators.
+ *   kind: 0 FFMA, 1 FFMA2 (packed f32x2), 2 DFMA, 3 MUFU.RSQ, 4 MUFU.RSQ64H, 5 FFMA2+MUFU in the force kernel's mix (12 : 2)
+ *   out4 (host) = { seconds, lane-operations executed, SM clock in MHz during the run, lane-ops/clk/SM }.
+ * Synchronous. */
+int pp_probe_pipe(int kind, int64_t iters, double* out4);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PPGRAV_H_ */

@@ -1,0 +1,213 @@
+// force_f32.cu -- FP32 all-pairs gravity sweep for sm_100a (the paper's "Gravity Force Computation" kernel,
+// PAPER.md:110-112, eq. (1)-(2) PAPER.md:41-48), redesigned for Blackwell:
+//
+//  * j-bodies arrive in shared memory through a 4-stage TMA bulk-copy ring (tma_ring.cuh); no thread spends
+//    issue slots on staging and warps only meet at mbarriers.
+//  * each thread keeps IPT i-bodies in registers and processes TWO j-bodies per instruction with the packed
+//    f32x2 pipe instructions sm_100 added (FADD2/FMUL2/FFMA2): the tile is stored pair-interleaved
+//    {x0 x1 y0 y1 z0 z1 m0 m1}, so one LDS.128 yields two ready-made packed operands.  Per pair of interactions:
+//    3 FADD2 + 3 FFMA2 + 2 MUFU.RSQ + 3 FMUL2 + 3 FFMA2 (+1 FADD2 with the potential) = 12 (13) FP32-pipe
+//    operations per interaction in 7 (7.5) issue slots.
+//  * accumulation is blocked: the packed accumulators only ever hold TJ/2 terms; after every tile they are folded
+//    into a compensated (TwoSum) FP32 outer sum.  A single FP32 accumulator over 2^20 terms is wrong at the 1e-3
+//    level; this keeps the whole solve at ~1e-7.
+//  * the (i-block, j-split) decomposition gives the 148 SMs an even number of equal work units at any N; partial
+//    sums go to a workspace and are added in fixed order by finalize (update.cu) -- no floating-point atomics.
+#include "ppgrav_internal.h"
+#include "tma_ring.cuh"
+
+namespace ppgrav {
+namespace {
+
+__device__ __forceinline__ float rsqrt_approx(float x) {
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// s + c += t with the rounding error of the addition captured in c (Knuth TwoSum; never contracted or reassociated)
+__device__ __forceinline__ void comp_add(float& s, float& c, float t) {
+    const float n = __fadd_rn(s, t);
+    const float bp = __fsub_rn(n, s);
+    const float e = __fadd_rn(__fsub_rn(s, __fsub_rn(n, bp)), __fsub_rn(t, bp));
+    s = n;
+    c = __fadd_rn(c, e);
+}
+
+template <int IPT, int MODE, bool GUARD, bool DIAG>
+__device__ __forceinline__ void sweep_tile(const float4* __restrict__ tp, const int npairs, const float2 (&nx)[IPT],
+                                           const float2 (&ny)[IPT], const float2 (&nz)[IPT], float2 (&ax)[IPT],
+                                           float2 (&ay)[IPT], float2 (&az)[IPT], float2 (&ap)[IPT], const float2 eps2,
+                                           const int jbase, const int (&iidx)[IPT]) {
+#pragma unroll 2
+    for (int p = 0; p < npairs; ++p) {
+        const float4 a = tp[2 * p];
+        const float4 b = tp[2 * p + 1];
+        const float2 xj = make_float2(a.x, a.y), yj = make_float2(a.z, a.w);
+        const float2 zj = make_float2(b.x, b.y), mj = make_float2(b.z, b.w);
+#pragma unroll
+        for (int k = 0; k < IPT; ++k) {
+            const float2 dx = __fadd2_rn(xj, nx[k]);          // r_j - r_i (two j-bodies)
+            const float2 dy = __fadd2_rn(yj, ny[k]);
+            const float2 dz = __fadd2_rn(zj, nz[k]);
+            float2 r2 = __ffma2_rn(dx, dx, eps2);             // |r_i - r_j|^2 + delta^2
+            r2 = __ffma2_rn(dy, dy, r2);
+            r2 = __ffma2_rn(dz, dz, r2);
+            float2 w;
+            w.x = rsqrt_approx(r2.x);
+            w.y = rsqrt_approx(r2.y);
+            if (GUARD) {                                      // delta == 0: zero-distance pairs contribute nothing
+                w.x = r2.x > 0.f ? w.x : 0.f;
+                w.y = r2.y > 0.f ? w.y : 0.f;
+            }
+            const float2 w2 = __fmul2_rn(w, w);
+            float2 mw = __fmul2_rn(mj, w);
+            const float2 s = __fmul2_rn(mw, w2);              // m_j / (r^2 + delta^2)^{3/2}
+            ax[k] = __ffma2_rn(s, dx, ax[k]);
+            ay[k] = __ffma2_rn(s, dy, ay[k]);
+            az[k] = __ffma2_rn(s, dz, az[k]);
+            if (MODE == MODE_FORCE_POT) {
+                if (DIAG) {                                   // tile overlaps this CTA's own bodies: drop j == i
+                    const int j0 = jbase + 2 * p;
+                    if (j0 == iidx[k]) mw.x = 0.f;
+                    if (j0 + 1 == iidx[k]) mw.y = 0.f;
+                }
+                ap[k] = __fadd2_rn(ap[k], mw);                // m_j / (r^2 + delta^2)^{1/2}
+            }
+        }
+    }
+}
+
+template <int THREADS, int IPT, int TJ, int STAGES, int MINB, int MODE, bool GUARD>
+__global__ void __launch_bounds__(THREADS, MINB)
+force_f32_kernel(const float* __restrict__ packed, float4* __restrict__ partial, const int n_tiles,
+                 const int64_t n_pad, const float eps2f) {
+    constexpr int NWARPS = THREADS / 32;
+    constexpr uint32_t TILE_BYTES = TJ * 16u;
+    __shared__ __align__(128) float tiles[STAGES][TJ * 4];
+    __shared__ __align__(8) uint64_t full_bar[STAGES];
+    __shared__ __align__(8) uint64_t empty_bar[STAGES];
+
+    const int tid = threadIdx.x;
+    const int ib = blockIdx.x;
+    const int split = gridDim.y, sidx = blockIdx.y;
+    const int t0 = (int)(((int64_t)n_tiles * sidx) / split);
+    const int t1 = (int)(((int64_t)n_tiles * (sidx + 1)) / split);
+    const int nt = t1 - t0;
+
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < STAGES; ++s) {
+            mbar_init(&full_bar[s], 1);
+            mbar_init(&empty_bar[s], NWARPS);
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+    if (tid == 0) {
+        const int pre = nt < STAGES ? nt : STAGES;
+        for (int s = 0; s < pre; ++s) {
+            mbar_expect_tx(&full_bar[s], TILE_BYTES);
+            tma_load_1d(&tiles[s][0], packed + (size_t)(t0 + s) * TJ * 4, TILE_BYTES, &full_bar[s]);
+        }
+    }
+
+    // this thread's i-bodies (negated and duplicated into both packed lanes)
+    float2 nx[IPT], ny[IPT], nz[IPT];
+    float2 ax[IPT], ay[IPT], az[IPT], ap[IPT];
+    float sx[IPT], sy[IPT], sz[IPT], sp[IPT], cx[IPT], cy[IPT], cz[IPT], cp[IPT];
+    int iidx[IPT];
+#pragma unroll
+    for (int k = 0; k < IPT; ++k) {
+        const int i = ib * (THREADS * IPT) + k * THREADS + tid;
+        iidx[k] = i;
+        const float* q = packed + (size_t)(i >> 1) * 8 + (i & 1);
+        const float xi = q[0], yi = q[2], zi = q[4];
+        nx[k] = make_float2(-xi, -xi);
+        ny[k] = make_float2(-yi, -yi);
+        nz[k] = make_float2(-zi, -zi);
+        ax[k] = ay[k] = az[k] = ap[k] = make_float2(0.f, 0.f);
+        sx[k] = sy[k] = sz[k] = sp[k] = 0.f;
+        cx[k] = cy[k] = cz[k] = cp[k] = 0.f;
+    }
+    const float2 eps2 = make_float2(eps2f, eps2f);
+    const int i_lo = ib * (THREADS * IPT), i_hi = i_lo + THREADS * IPT;
+
+    for (int t = 0; t < nt; ++t) {
+        const int s = t % STAGES;
+        mbar_wait(&full_bar[s], (uint32_t)(t / STAGES) & 1u);
+        const float4* tp = reinterpret_cast<const float4*>(&tiles[s][0]);
+        const int jbase = (t0 + t) * TJ;
+        const bool diag = (MODE == MODE_FORCE_POT) && !GUARD && (jbase < i_hi) && (jbase + TJ > i_lo);
+        if (diag)
+            sweep_tile<IPT, MODE, GUARD, true>(tp, TJ / 2, nx, ny, nz, ax, ay, az, ap, eps2, jbase, iidx);
+        else
+            sweep_tile<IPT, MODE, GUARD, false>(tp, TJ / 2, nx, ny, nz, ax, ay, az, ap, eps2, jbase, iidx);
+
+        // release the stage, then (one tile late, so the wait is normally already satisfied) refill the stage
+        // that held tile t-1 with tile t-1+STAGES
+        __syncwarp();
+        if ((tid & 31) == 0) mbar_arrive(&empty_bar[s]);
+        if (tid == 0 && t >= 1 && t - 1 + STAGES < nt) {
+            const int ps = (t - 1) % STAGES;
+            mbar_wait(&empty_bar[ps], (uint32_t)((t - 1) / STAGES) & 1u);
+            mbar_expect_tx(&full_bar[ps], TILE_BYTES);
+            tma_load_1d(&tiles[ps][0], packed + (size_t)(t0 + t - 1 + STAGES) * TJ * 4, TILE_BYTES, &full_bar[ps]);
+        }
+
+        // blocked accumulation: fold the tile's packed partial sums into the compensated outer sums
+#pragma unroll
+        for (int k = 0; k < IPT; ++k) {
+            comp_add(sx[k], cx[k], __fadd_rn(ax[k].x, ax[k].y));
+            comp_add(sy[k], cy[k], __fadd_rn(ay[k].x, ay[k].y));
+            comp_add(sz[k], cz[k], __fadd_rn(az[k].x, az[k].y));
+            ax[k] = ay[k] = az[k] = make_float2(0.f, 0.f);
+            if (MODE == MODE_FORCE_POT) {
+                comp_add(sp[k], cp[k], __fadd_rn(ap[k].x, ap[k].y));
+                ap[k] = make_float2(0.f, 0.f);
+            }
+        }
+    }
+
+#pragma unroll
+    for (int k = 0; k < IPT; ++k) {
+        float4 o;
+        o.x = __fadd_rn(sx[k], cx[k]);
+        o.y = __fadd_rn(sy[k], cy[k]);
+        o.z = __fadd_rn(sz[k], cz[k]);
+        o.w = (MODE == MODE_FORCE_POT) ? __fadd_rn(sp[k], cp[k]) : 0.f;
+        partial[(size_t)sidx * n_pad + iidx[k]] = o;
+    }
+}
+
+template <int THREADS, int IPT, int TJ, int STAGES, int MINB>
+int launch_variant(const Plan& p, const float* packed, float4* partial, int64_t N, float eps2, bool guard, int mode,
+                   cudaStream_t st) {
+    const int n_ib = (int)((N + p.i_per_cta - 1) / p.i_per_cta);
+    dim3 grid(n_ib, p.split);
+#define PP_LAUNCH32(MODE_, GUARD_)                                                      \
+    force_f32_kernel<THREADS, IPT, TJ, STAGES, MINB, MODE_, GUARD_>                     \
+        <<<grid, THREADS, 0, st>>>(packed, partial, p.n_tiles, p.n_pad, eps2)
+    if (mode == MODE_FORCE) {
+        if (guard) PP_LAUNCH32(MODE_FORCE, true); else PP_LAUNCH32(MODE_FORCE, false);
+    } else {
+        if (guard) PP_LAUNCH32(MODE_FORCE_POT, true); else PP_LAUNCH32(MODE_FORCE_POT, false);
+    }
+#undef PP_LAUNCH32
+    count_launch();
+    PP_CUDA(cudaGetLastError());
+    return PP_OK;
+}
+
+}  // namespace
+
+int launch_force_f32(const Plan& p, const float* packed, float4* partial, int64_t N, double delta, int mode,
+                     cudaStream_t st) {
+    const float eps2 = (float)(delta * delta);
+    // guarded variant whenever delta^2 is not a normal positive float (r^2 could then be exactly 0)
+    const bool guard = !(eps2 >= 1.17549435e-38f);
+    if (p.variant == 0) return launch_variant<256, 4, 256, 4, 2>(p, packed, partial, N, eps2, guard, mode, st);
+    return launch_variant<128, 1, 128, 4, 4>(p, packed, partial, N, eps2, guard, mode, st);
+}
+
+}  // namespace ppgrav

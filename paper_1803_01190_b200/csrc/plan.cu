@@ -1,0 +1,71 @@
+// plan.cu -- host-side launch plan of one gravity solve (no device code).
+//
+// The all-pairs sweep of eq. (1) is cut into (i-block, j-split) work units.  The paper's Kepler GPUs
+// had 13-15 SMs, so "one thread per i-particle" filled them at any N of interest; a B200 has 148 SMs
+// and N = 2^20 bodies in 1024-body i-blocks are only 3.5 waves.  The plan therefore picks the kernel variant and the
+// split factor S that minimise  waves x (tiles per split + fixed overhead)  so that the last wave is nearly full.
+#include <algorithm>
+
+#include "ppgrav_internal.h"
+
+namespace ppgrav {
+
+namespace {
+
+struct VariantDesc {
+    int threads, ipt, tile_j, stages, ctas_per_sm;
+    double eff;   // relative pair throughput of one SM running this variant (variant 0 = 1)
+};
+
+// must match the template instantiations in force_f32.cu / force_f64.cu
+const VariantDesc kVariants[2][2] = {
+    /* PP_F32 */ {{256, 4, 256, 4, 2, 1.0}, {128, 1, 128, 4, 4, 0.45}},
+    /* PP_F64 */ {{256, 4, 256, 4, 1, 1.0}, {128, 1, 128, 4, 4, 0.80}},
+};
+
+int64_t round_up(int64_t a, int64_t b) { return (a + b - 1) / b * b; }
+
+}  // namespace
+
+Plan make_plan(int64_t N, int precision, int sm_count, int64_t forced_split) {
+    Plan best{};
+    double best_cost = -1.0;
+    const size_t elem = precision == PP_F64 ? 32 : 16;
+    for (int v = 0; v < 2; ++v) {
+        const VariantDesc& d = kVariants[precision == PP_F64 ? 1 : 0][v];
+        Plan p{};
+        p.variant = v;
+        p.threads = d.threads;
+        p.ipt = d.ipt;
+        p.i_per_cta = d.threads * d.ipt;
+        p.tile_j = d.tile_j;
+        p.stages = d.stages;
+        p.ctas_per_sm = d.ctas_per_sm;
+        p.sm_count = sm_count;
+        p.n_pad = round_up(N, std::max(p.i_per_cta, p.tile_j));   // tile_j divides i_per_cta in both variants
+        p.n_iblocks = (int)((N + p.i_per_cta - 1) / p.i_per_cta);
+        p.n_tiles = (int)((N + p.tile_j - 1) / p.tile_j);
+        const int64_t resident = (int64_t)sm_count * d.ctas_per_sm;
+        // partial sums: S x n_pad x {16,32} bytes, kept under 1 GiB
+        int64_t s_max = std::min<int64_t>(std::min<int64_t>(p.n_tiles, 64),
+                                          std::max<int64_t>(1, (int64_t)((1ull << 30) / (p.n_pad * elem))));
+        int64_t s_lo = 1, s_hi = s_max;
+        if (forced_split >= 1) s_lo = s_hi = std::min<int64_t>(forced_split, p.n_tiles);
+        const double tile_cost = (double)p.i_per_cta * p.tile_j * d.ctas_per_sm / d.eff;
+        for (int64_t S = s_lo; S <= s_hi; ++S) {
+            const int64_t units = (int64_t)p.n_iblocks * S;
+            const int64_t waves = (units + resident - 1) / resident;
+            const int64_t tps = (p.n_tiles + S - 1) / S;
+            // 2 tile-times of fixed cost per unit (pipeline fill, epilogue), plus the finalize pass over S partials
+            const double cost = (double)waves * ((double)tps + 2.0) * tile_cost + 64.0 * (double)S * (double)p.n_pad;
+            if (best_cost < 0.0 || cost < best_cost * (1.0 - 1e-9)) {
+                best_cost = cost;
+                best = p;
+                best.split = (int)S;
+            }
+        }
+    }
+    return best;
+}
+
+}  // namespace ppgrav

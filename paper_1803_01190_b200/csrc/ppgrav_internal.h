@@ -1,0 +1,84 @@
+// ppgrav_internal.h -- declarations shared by the translation units of libppgrav (not part of the C ABI).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "ppgrav.h"
+
+namespace ppgrav {
+
+// ---- error plumbing (api.cu) ------------------------------------------------------------------------------
+void set_error(const char* fmt, ...);
+int cuda_fail(cudaError_t e, const char* what);   // records the message, returns PP_ECUDA
+void count_launch(int n = 1);
+
+#define PP_CUDA(call)                                            \
+    do {                                                         \
+        cudaError_t e__ = (call);                                \
+        if (e__ != cudaSuccess) return ::ppgrav::cuda_fail(e__, #call); \
+    } while (0)
+
+// ---- launch plan of one gravity solve (plan.cu) --------------------------------------------------------------
+// The all-pairs sweep is cut into work units (i-block, j-split): CTA (ib, s) sweeps the j-tiles of split s for the
+// bodies of i-block ib and writes one partial sum per body; a finalize kernel adds the S partials in fixed order.
+struct Plan {
+    int variant;        // 0 = large (256 threads x 4 i-bodies), 1 = small (128 threads x 1 i-body)
+    int threads;        // threads per CTA
+    int ipt;            // i-bodies per thread
+    int i_per_cta;      // threads * ipt
+    int tile_j;         // j-bodies per shared-memory tile
+    int stages;         // depth of the TMA ring
+    int ctas_per_sm;    // residency the kernel is built for
+    int64_t n_pad;      // N rounded up to a multiple of lcm(i_per_cta, tile_j): length of the packed array
+    int n_iblocks;      // n_pad / i_per_cta (only blocks that contain a real body are launched)
+    int n_tiles;        // ceil(N / tile_j): j-tiles that contain a real body
+    int split;          // S
+    int sm_count;
+};
+Plan make_plan(int64_t N, int precision, int sm_count, int64_t forced_split);
+
+// modes of the pair sweep
+enum { MODE_FORCE = 0, MODE_FORCE_POT = 1, MODE_POT = 2 };
+
+// ---- kernels (one launcher per translation unit) -----------------------------------------------------------------
+// Packed bodies.  FP32: pairs of bodies interleaved, 8 floats {x0 x1 y0 y1 z0 z1 m0 m1} per pair (so that one
+// 64-bit shared-memory word feeds one packed f32x2 operand).  FP64: double4 {x y z m} per body.  Bodies N..n_pad-1
+// are padding: mass 0 at the origin.
+int launch_pack_f32(const float* pos, const float* mass, float* packed, int64_t N, int64_t n_pad, cudaStream_t st);
+int launch_pack_f64(const double* pos, const double* mass, double* packed, int64_t N, int64_t n_pad, cudaStream_t st);
+int launch_pack_f32_to_f64(const float* pos, const float* mass, double* packed, int64_t N, int64_t n_pad,
+                           cudaStream_t st);
+
+// partial[s * n_pad + i] = {sum_x, sum_y, sum_z, sum_pot} over the j-tiles of split s, without G and with the
+// sign convention  sum = sum_j m_j (r_j - r_i) w^3,  sum_pot = sum_j m_j w   (w = (r^2+delta^2)^{-1/2}).
+int launch_force_f32(const Plan& p, const float* packed, float4* partial, int64_t N, double delta, int mode,
+                     cudaStream_t st);
+// MODE_POT writes {pot_hi, pot_lo, 0, 0} (double-double partial of the potential sum).
+int launch_force_f64(const Plan& p, const double* packed, double4* partial, int64_t N, double delta, int mode,
+                     cudaStream_t st);
+
+// acc = G * sum_s partial (fixed order, compensated), pot = -G * sum_s partial.w; optional fused kick
+// vel += kick * acc (kick = 0: none).  acc/pot/vel may be NULL where not wanted.
+int launch_finalize_f32(const float4* partial, int split, int64_t n_pad, int64_t N, double G, float* acc, float* pot,
+                        float* vel, double kick, cudaStream_t st);
+int launch_finalize_f64(const double4* partial, int split, int64_t n_pad, int64_t N, double G, double* acc,
+                        double* pot, double* vel, double kick, int pot_is_dd, cudaStream_t st);
+
+// v += kick * a;  r += dt * v;  packed = pack(r, m)      (eqs. (5)-(6) in half-kick form)
+int launch_kick_drift_pack_f32(float* pos, float* vel, const float* acc, const float* mass, float* packed, int64_t N,
+                               int64_t n_pad, double kick, double dt, cudaStream_t st);
+int launch_kick_drift_pack_f64(double* pos, double* vel, const double* acc, const double* mass, double* packed,
+                               int64_t N, int64_t n_pad, double kick, double dt, cudaStream_t st);
+
+// eqs. (8)-(10): block partials (double-double) then a single-block fixed-order sum into out16.
+int invariants_scratch_doubles(int64_t N);
+int launch_invariants_f32(const float* pos, const float* vel, const float* mass, const float* pot_state,
+                          const double* pot64, int64_t N, double* scratch, double* out16, cudaStream_t st);
+int launch_invariants_f64(const double* pos, const double* vel, const double* mass, const double* pot_state,
+                          const double* pot64, int64_t N, double* scratch, double* out16, cudaStream_t st);
+
+// pipe microbenchmarks (probe.cu)
+int run_probe(int kind, int64_t iters, int sm_count, double* out4);
+
+}  // namespace ppgrav

@@ -1,0 +1,182 @@
+// probe.cu -- pipe-throughput microbenchmarks: the MEASURED denominators of the ALU roofline.
+//
+// The force kernels are bound by the FP32 / FP64 pipes, not by HBM or tensor cores, and MEASURED_PEAKS.json holds
+// no CUDA-core peak.  Each probe runs a long, register-only dependent-chain loop (8 independent chains per thread,
+// 32 warps per SM) of one instruction kind and reports lane-operations per clock per SM, with the SM clock taken
+// from clock64()/globaltimer inside the kernel.
+#include "ppgrav_internal.h"
+
+namespace ppgrav {
+namespace {
+
+constexpr int kThreads = 256;
+constexpr int kCtasPerSm = 4;
+constexpr int kChains = 8;
+constexpr int kInner = 8;
+
+__device__ __forceinline__ uint64_t globaltimer_ns() {
+    uint64_t t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+__device__ __forceinline__ float rsqrt_f32(float x) {
+    float y;
+    asm volatile("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ double rsqrt_f64h(double x) {
+    double y;
+    asm volatile("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    return y;
+}
+
+// KIND: 0 FFMA, 1 FFMA2, 2 DFMA, 3 MUFU.RSQ, 4 MUFU.RSQ64H, 5 the force kernel's mix (12 FFMA2 : 2 MUFU.RSQ = two pairs)
+template <int KIND>
+__global__ void __launch_bounds__(kThreads, kCtasPerSm)
+probe_kernel(int64_t iters, float seed, float* __restrict__ sink, uint64_t* __restrict__ clk) {
+    const uint64_t t0 = globaltimer_ns();
+    const long long c0 = clock64();
+    float acc = 0.f;
+    if (KIND == 0) {
+        float a[kChains];
+        const float b = 1.0f + (seed + threadIdx.x) * 1e-9f, c = (seed + threadIdx.x) * 1e-9f;   // per-thread: 3-register form
+#pragma unroll
+        for (int k = 0; k < kChains; ++k) a[k] = seed + k + threadIdx.x;
+        for (int64_t it = 0; it < iters; ++it)
+#pragma unroll
+            for (int u = 0; u < kInner; ++u)
+#pragma unroll
+                for (int k = 0; k < kChains; ++k) a[k] = __fmaf_rn(a[k], b, c);
+#pragma unroll
+        for (int k = 0; k < kChains; ++k) acc += a[k];
+    } else if (KIND == 1) {
+        float2 a[kChains];
+        const float tx = (seed + threadIdx.x) * 1e-9f;
+        const float2 b = make_float2(1.0f + tx, 1.0f - tx), c = make_float2(tx, seed + tx);
+#pragma unroll
+        for (int k = 0; k < kChains; ++k) a[k] = make_float2(seed + k, seed + threadIdx.x);
+        for (int64_t it = 0; it < iters; ++it)
+#pragma unroll
+            for (int u = 0; u < kInner; ++u)
+#pragma unroll
+                for (int k = 0; k < kChains; ++k) a[k] = __ffma2_rn(a[k], b, c);
+#pragma unroll
+        for (int k = 0; k < kChains; ++k) acc += a[k].x + a[k].y;
+    } else if (KIND == 2) {
+        double a[kChains];
+        const double b = 1.0 + (seed + threadIdx.x) * 1e-12, c = (seed + threadIdx.x) * 1e-12;
+#pragma unroll
+        for (int k = 0; k < kChains; ++k) a[k] = seed + k + threadIdx.x;
+        for (int64_t it = 0; it < iters; ++it)
+#pragma unroll
+            for (int u = 0; u < kInner; ++u)
+#pragma unroll
+                for (int k = 0; k < kChains; ++k) a[k] = __fma_rn(a[k], b, c);
+#pragma unroll
+        for (int k = 0; k < kChains; ++k) acc += (float)a[k];
+    } else if (KIND == 3) {
+        float a[kChains];
+#pragma unroll
+        for (int k = 0; k < kChains; ++k) a[k] = 1.0f + seed + k + threadIdx.x;
+        for (int64_t it = 0; it < iters; ++it)
+#pragma unroll
+            for (int u = 0; u < kInner; ++u)
+#pragma unroll
+                for (int k = 0; k < kChains; ++k) a[k] = rsqrt_f32(a[k]);
+#pragma unroll
+        for (int k = 0; k < kChains; ++k) acc += a[k];
+    } else if (KIND == 4) {
+        double a[kChains];
+#pragma unroll
+        for (int k = 0; k < kChains; ++k) a[k] = 1.0 + seed + k + threadIdx.x;
+        for (int64_t it = 0; it < iters; ++it)
+#pragma unroll
+            for (int u = 0; u < kInner; ++u)
+#pragma unroll
+                for (int k = 0; k < kChains; ++k) a[k] = rsqrt_f64h(a[k]);
+#pragma unroll
+        for (int k = 0; k < kChains; ++k) acc += (float)a[k];
+    } else {
+        float2 a[kChains];
+        const float tx = (seed + threadIdx.x) * 1e-9f;
+        const float2 b = make_float2(1.0f + tx, 1.0f - tx), c = make_float2(1.0f + tx, 1.0f + seed);
+#pragma unroll
+        for (int k = 0; k < kChains; ++k) a[k] = make_float2(1.0f + seed + k, 1.0f + threadIdx.x);
+        for (int64_t it = 0; it < iters; ++it)
+#pragma unroll
+            for (int u = 0; u < kInner; ++u)
+#pragma unroll
+                for (int k = 0; k < kChains; ++k) {
+                    float2 r = a[k];
+#pragma unroll
+                    for (int f = 0; f < 12; ++f) r = __ffma2_rn(r, b, c);
+                    a[k] = make_float2(rsqrt_f32(r.x), rsqrt_f32(r.y));
+                }
+#pragma unroll
+        for (int k = 0; k < kChains; ++k) acc += a[k].x + a[k].y;
+    }
+    const long long c1 = clock64();
+    const uint64_t t1 = globaltimer_ns();
+    if (acc == 123.456f) sink[0] = acc;   // keeps the chains alive; practically never true
+    if (threadIdx.x == 0) {
+        clk[2 * blockIdx.x] = (uint64_t)(c1 - c0);
+        clk[2 * blockIdx.x + 1] = t1 - t0;
+    }
+}
+
+template <int KIND>
+void launch(int grid, int64_t iters, float* sink, uint64_t* clk) {
+    probe_kernel<KIND><<<grid, kThreads>>>(iters, 0.5f, sink, clk);
+}
+
+}  // namespace
+
+int run_probe(int kind, int64_t iters, int sm_count, double* out4) {
+    if (kind < 0 || kind > 5 || iters < 1) {
+        set_error("pp_probe_pipe: kind must be 0..5 and iters >= 1");
+        return PP_EINVAL;
+    }
+    const int grid = sm_count * kCtasPerSm;
+    float* sink = nullptr;
+    uint64_t* clk = nullptr;
+    PP_CUDA(cudaMalloc(&sink, 4));
+    PP_CUDA(cudaMalloc(&clk, sizeof(uint64_t) * 2 * grid));
+    cudaEvent_t e0, e1;
+    PP_CUDA(cudaEventCreate(&e0));
+    PP_CUDA(cudaEventCreate(&e1));
+    float ms = 0.f;
+    for (int rep = 0; rep < 2; ++rep) {   // first repetition warms up clocks and the instruction cache
+        PP_CUDA(cudaEventRecord(e0));
+        switch (kind) {
+            case 0: launch<0>(grid, iters, sink, clk); break;
+            case 1: launch<1>(grid, iters, sink, clk); break;
+            case 2: launch<2>(grid, iters, sink, clk); break;
+            case 3: launch<3>(grid, iters, sink, clk); break;
+            case 4: launch<4>(grid, iters, sink, clk); break;
+            default: launch<5>(grid, iters, sink, clk); break;
+        }
+        count_launch();
+        PP_CUDA(cudaGetLastError());
+        PP_CUDA(cudaEventRecord(e1));
+        PP_CUDA(cudaEventSynchronize(e1));
+        PP_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+    }
+    uint64_t h[2];
+    PP_CUDA(cudaMemcpy(h, clk, sizeof(h), cudaMemcpyDeviceToHost));
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(sink);
+    cudaFree(clk);
+    // lane-operations per chain step: packed instructions count 2 lanes; the mix counts its 12 FFMA2 (24 lane-ops)
+    const double per_step = (kind == 1) ? 2.0 : (kind == 5) ? 24.0 : 1.0;
+    const double lane_ops = (double)grid * kThreads * (double)iters * kInner * kChains * per_step;
+    const double sec = ms * 1e-3;
+    const double mhz = h[1] ? (double)h[0] / (double)h[1] * 1e3 : 0.0;
+    out4[0] = sec;
+    out4[1] = lane_ops;
+    out4[2] = mhz;
+    out4[3] = (mhz > 0.0) ? lane_ops / (sec * mhz * 1e6 * sm_count) : 0.0;
+    return PP_OK;
+}
+
+}  // namespace ppgrav

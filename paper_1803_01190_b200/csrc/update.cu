@@ -1,0 +1,169 @@
+// update.cu -- the O(N) kernels around the gravity solve: packing, split-j finalize, and the paper's "Update
+// System" kernel in half-kick form (eqs. (5)-(7); reading R4).
+//
+// All of them are HBM-bound element-wise passes (<= 200 B per body per step against >= N x 12 pipe operations per
+// body in the force kernel), so they are written for coalescing and fusion, not for arithmetic:
+//   pack            pos[N,3], mass[N] -> packed tile layout (float pairs interleaved / double4), padding included
+//   finalize        acc = G sum_s partial[s] (fixed order, compensated) [, pot = -G sum_s] [, vel += kick acc]
+//   kick_drift_pack vel += kick acc; pos += dt vel; packed = pack(pos, mass)   -- one pass instead of three
+#include "ppgrav_internal.h"
+
+namespace ppgrav {
+namespace {
+
+constexpr int kThreads = 256;
+
+inline int grid_for(int64_t n) { return (int)((n + kThreads - 1) / kThreads); }
+
+// FP32 packed layout: body i lives in pair i>>1, lane i&1 of {x0 x1 y0 y1 z0 z1 m0 m1}
+__device__ __forceinline__ void store_packed(float* packed, int64_t i, float x, float y, float z, float m) {
+    float* q = packed + (i >> 1) * 8 + (i & 1);
+    q[0] = x; q[2] = y; q[4] = z; q[6] = m;
+}
+__device__ __forceinline__ void store_packed(double* packed, int64_t i, double x, double y, double z, double m) {
+    reinterpret_cast<double4*>(packed)[i] = make_double4(x, y, z, m);
+}
+
+template <typename TIn, typename TOut>
+__global__ void __launch_bounds__(kThreads) pack_kernel(const TIn* __restrict__ pos, const TIn* __restrict__ mass,
+                                                        TOut* __restrict__ packed, int64_t N, int64_t n_pad) {
+    const int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x;
+    if (i >= n_pad) return;
+    if (i < N)
+        store_packed(packed, i, (TOut)pos[3 * i], (TOut)pos[3 * i + 1], (TOut)pos[3 * i + 2], (TOut)mass[i]);
+    else
+        store_packed(packed, i, (TOut)0, (TOut)0, (TOut)0, (TOut)0);   // padding: massless, contributes nothing
+}
+
+// error-free s + t -> (s, err accumulated into c); intrinsics keep the compiler from contracting/reassociating
+__device__ __forceinline__ void comp_add(float& s, float& c, float t) {
+    const float n = __fadd_rn(s, t);
+    const float bp = __fsub_rn(n, s);
+    c = __fadd_rn(c, __fadd_rn(__fsub_rn(s, __fsub_rn(n, bp)), __fsub_rn(t, bp)));
+    s = n;
+}
+__device__ __forceinline__ void comp_add(double& s, double& c, double t) {
+    const double n = __dadd_rn(s, t);
+    const double bp = __dsub_rn(n, s);
+    c = __dadd_rn(c, __dadd_rn(__dsub_rn(s, __dsub_rn(n, bp)), __dsub_rn(t, bp)));
+    s = n;
+}
+
+template <typename T> struct Vec4;
+template <> struct Vec4<float> { using type = float4; };
+template <> struct Vec4<double> { using type = double4; };
+
+// POT_DD: partial.x/.y are the hi/lo words of a double-double potential sum (MODE_POT of force_f64.cu)
+template <typename T, bool POT_DD>
+__global__ void __launch_bounds__(kThreads)
+finalize_kernel(const typename Vec4<T>::type* __restrict__ partial, int split, int64_t n_pad, int64_t N, T G,
+                T* __restrict__ acc, T* __restrict__ pot, T* __restrict__ vel, T kick) {
+    const int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x;
+    if (i >= N) return;
+    T sx = 0, sy = 0, sz = 0, sw = 0, cx = 0, cy = 0, cz = 0, cw = 0;
+    for (int s = 0; s < split; ++s) {   // fixed order s = 0..S-1: run-to-run deterministic
+        const typename Vec4<T>::type v = partial[(size_t)s * n_pad + i];
+        if (POT_DD) {
+            comp_add(sx, cx, v.x);
+            comp_add(sx, cx, v.y);
+        } else {
+            comp_add(sx, cx, v.x);
+            comp_add(sy, cy, v.y);
+            comp_add(sz, cz, v.z);
+            comp_add(sw, cw, v.w);
+        }
+    }
+    if (POT_DD) {
+        if (pot) pot[i] = -G * (sx + cx);
+        return;
+    }
+    const T ax = G * (sx + cx), ay = G * (sy + cy), az = G * (sz + cz);
+    if (acc) { acc[3 * i] = ax; acc[3 * i + 1] = ay; acc[3 * i + 2] = az; }
+    if (pot) pot[i] = -G * (sw + cw);
+    if (vel) {   // closing half-kick of eq. (7): v(t+dt) = v~ + dt/2 a(t+dt)
+        vel[3 * i] = fma(kick, ax, vel[3 * i]);
+        vel[3 * i + 1] = fma(kick, ay, vel[3 * i + 1]);
+        vel[3 * i + 2] = fma(kick, az, vel[3 * i + 2]);
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(kThreads)
+kick_drift_pack_kernel(T* __restrict__ pos, T* __restrict__ vel, const T* __restrict__ acc,
+                       const T* __restrict__ mass, T* __restrict__ packed, int64_t N, int64_t n_pad, T kick, T dt) {
+    const int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x;
+    if (i >= n_pad) return;
+    if (i >= N) { store_packed(packed, i, (T)0, (T)0, (T)0, (T)0); return; }
+    T r[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const T v = fma(kick, acc[3 * i + c], vel[3 * i + c]);   // opening half-kick, eq. (5) halved
+        vel[3 * i + c] = v;
+        r[c] = fma(dt, v, pos[3 * i + c]);                       // drift, eq. (6)
+        pos[3 * i + c] = r[c];
+    }
+    store_packed(packed, i, r[0], r[1], r[2], mass[i]);
+}
+
+}  // namespace
+
+int launch_pack_f32(const float* pos, const float* mass, float* packed, int64_t N, int64_t n_pad, cudaStream_t st) {
+    pack_kernel<float, float><<<grid_for(n_pad), kThreads, 0, st>>>(pos, mass, packed, N, n_pad);
+    count_launch();
+    PP_CUDA(cudaGetLastError());
+    return PP_OK;
+}
+int launch_pack_f64(const double* pos, const double* mass, double* packed, int64_t N, int64_t n_pad,
+                    cudaStream_t st) {
+    pack_kernel<double, double><<<grid_for(n_pad), kThreads, 0, st>>>(pos, mass, packed, N, n_pad);
+    count_launch();
+    PP_CUDA(cudaGetLastError());
+    return PP_OK;
+}
+int launch_pack_f32_to_f64(const float* pos, const float* mass, double* packed, int64_t N, int64_t n_pad,
+                           cudaStream_t st) {
+    pack_kernel<float, double><<<grid_for(n_pad), kThreads, 0, st>>>(pos, mass, packed, N, n_pad);
+    count_launch();
+    PP_CUDA(cudaGetLastError());
+    return PP_OK;
+}
+
+int launch_finalize_f32(const float4* partial, int split, int64_t n_pad, int64_t N, double G, float* acc, float* pot,
+                        float* vel, double kick, cudaStream_t st) {
+    finalize_kernel<float, false><<<grid_for(N), kThreads, 0, st>>>(partial, split, n_pad, N, (float)G, acc, pot,
+                                                                    kick != 0.0 ? vel : nullptr, (float)kick);
+    count_launch();
+    PP_CUDA(cudaGetLastError());
+    return PP_OK;
+}
+int launch_finalize_f64(const double4* partial, int split, int64_t n_pad, int64_t N, double G, double* acc,
+                        double* pot, double* vel, double kick, int pot_is_dd, cudaStream_t st) {
+    if (pot_is_dd)
+        finalize_kernel<double, true><<<grid_for(N), kThreads, 0, st>>>(partial, split, n_pad, N, G, nullptr, pot,
+                                                                        nullptr, 0.0);
+    else
+        finalize_kernel<double, false><<<grid_for(N), kThreads, 0, st>>>(partial, split, n_pad, N, G, acc, pot,
+                                                                         kick != 0.0 ? vel : nullptr, kick);
+    count_launch();
+    PP_CUDA(cudaGetLastError());
+    return PP_OK;
+}
+
+int launch_kick_drift_pack_f32(float* pos, float* vel, const float* acc, const float* mass, float* packed, int64_t N,
+                               int64_t n_pad, double kick, double dt, cudaStream_t st) {
+    kick_drift_pack_kernel<float><<<grid_for(n_pad), kThreads, 0, st>>>(pos, vel, acc, mass, packed, N, n_pad,
+                                                                        (float)kick, (float)dt);
+    count_launch();
+    PP_CUDA(cudaGetLastError());
+    return PP_OK;
+}
+int launch_kick_drift_pack_f64(double* pos, double* vel, const double* acc, const double* mass, double* packed,
+                               int64_t N, int64_t n_pad, double kick, double dt, cudaStream_t st) {
+    kick_drift_pack_kernel<double><<<grid_for(n_pad), kThreads, 0, st>>>(pos, vel, acc, mass, packed, N, n_pad, kick,
+                                                                         dt);
+    count_launch();
+    PP_CUDA(cudaGetLastError());
+    return PP_OK;
+}
+
+}  // namespace ppgrav
