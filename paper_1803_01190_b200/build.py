@@ -32,13 +32,15 @@ def _stale():
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force=False, verbose=False):
-    """Compile every translation unit and link paper_1803_01190_b200/libppgrav.so.  Returns its path."""
-    if not force and not _stale():
+def build(force=False, verbose=False, extra_flags=(), out=None):
+    """Compile every translation unit and link paper_1803_01190_b200/libppgrav.so.  Returns its path.
+    extra_flags / out: tuning builds with -DPP_F32_IPT=... shape overrides into another file."""
+    if out is None and not force and not _stale():
         return LIB
-    objdir = os.path.join(HERE, "build")
+    objdir = os.path.join(HERE, "build") if out is None else out + ".objs"
+    out = LIB if out is None else out
     os.makedirs(objdir, exist_ok=True)
-    flags = list(NVCC_FLAGS) + (["-Xptxas", "-v"] if verbose else [])
+    flags = list(NVCC_FLAGS) + list(extra_flags) + (["-Xptxas", "-v"] if verbose else [])
     procs = []
     for src in SOURCES:
         obj = os.path.join(objdir, src.replace(".cu", ".o"))
@@ -46,15 +48,15 @@ def build(force=False, verbose=False):
         procs.append((src, obj, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
     objs = []
     for src, obj, p in procs:
-        out, _ = p.communicate()
+        log, _ = p.communicate()
         if verbose or p.returncode != 0:
-            sys.stderr.write(out)
+            sys.stderr.write(log)
         if p.returncode != 0:
             raise RuntimeError("nvcc failed on %s" % src)
         objs.append(obj)
-    cmd = [_nvcc(), "-shared", "-o", LIB] + objs + ["-gencode", "arch=compute_100a,code=sm_100a", "-lcudart"]
+    cmd = [_nvcc(), "-shared", "-o", out] + objs + ["-gencode", "arch=compute_100a,code=sm_100a", "-lcudart"]
     subprocess.run(cmd, check=True)
-    return LIB
+    return out
 
 
 if __name__ == "__main__":

@@ -39,7 +39,7 @@ __device__ __forceinline__ void sweep_tile(const float4* __restrict__ tp, const 
                                            const float2 (&ny)[IPT], const float2 (&nz)[IPT], float2 (&ax)[IPT],
                                            float2 (&ay)[IPT], float2 (&az)[IPT], float2 (&ap)[IPT], const float2 eps2,
                                            const int jbase, const int (&iidx)[IPT]) {
-#pragma unroll 2
+#pragma unroll kF32Unroll
     for (int p = 0; p < npairs; ++p) {
         const float4 a = tp[2 * p];
         const float4 b = tp[2 * p + 1];
@@ -206,8 +206,12 @@ int launch_force_f32(const Plan& p, const float* packed, float4* partial, int64_
     const float eps2 = (float)(delta * delta);
     // guarded variant whenever delta^2 is not a normal positive float (r^2 could then be exactly 0)
     const bool guard = !(eps2 >= 1.17549435e-38f);
-    if (p.variant == 0) return launch_variant<256, 4, 256, 4, 2>(p, packed, partial, N, eps2, guard, mode, st);
-    return launch_variant<128, 1, 128, 4, 4>(p, packed, partial, N, eps2, guard, mode, st);
+    constexpr KernelShape L = kShapeF32Large, S = kShapeF32Small;
+    if (p.variant == 0)
+        return launch_variant<L.threads, L.ipt, L.tile_j, L.stages, L.ctas_per_sm>(p, packed, partial, N, eps2, guard,
+                                                                                    mode, st);
+    return launch_variant<S.threads, S.ipt, S.tile_j, S.stages, S.ctas_per_sm>(p, packed, partial, N, eps2, guard,
+                                                                                mode, st);
 }
 
 }  // namespace ppgrav

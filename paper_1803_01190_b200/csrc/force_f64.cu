@@ -36,7 +36,7 @@ __device__ __forceinline__ void sweep_tile(const double4* __restrict__ tp, const
                                            const double (&yi)[IPT], const double (&zi)[IPT], double (&ax)[IPT],
                                            double (&ay)[IPT], double (&az)[IPT], double (&ap)[IPT], const double eps2,
                                            const int jbase, const int (&iidx)[IPT]) {
-#pragma unroll 2
+#pragma unroll kF64Unroll
     for (int j = 0; j < nj; ++j) {
         const double4 b = tp[j];
 #pragma unroll
@@ -194,8 +194,12 @@ int launch_force_f64(const Plan& p, const double* packed, double4* partial, int6
                      cudaStream_t st) {
     const double eps2 = delta * delta;
     const bool guard = !(eps2 >= 2.2250738585072014e-308);
-    if (p.variant == 0) return launch_variant<256, 4, 256, 4, 1>(p, packed, partial, N, eps2, guard, mode, st);
-    return launch_variant<128, 1, 128, 4, 4>(p, packed, partial, N, eps2, guard, mode, st);
+    constexpr KernelShape L = kShapeF64Large, S = kShapeF64Small;
+    if (p.variant == 0)
+        return launch_variant<L.threads, L.ipt, L.tile_j, L.stages, L.ctas_per_sm>(p, packed, partial, N, eps2, guard,
+                                                                                    mode, st);
+    return launch_variant<S.threads, S.ipt, S.tile_j, S.stages, S.ctas_per_sm>(p, packed, partial, N, eps2, guard,
+                                                                                mode, st);
 }
 
 }  // namespace ppgrav

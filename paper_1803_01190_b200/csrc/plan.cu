@@ -13,14 +13,13 @@ namespace ppgrav {
 namespace {
 
 struct VariantDesc {
-    int threads, ipt, tile_j, stages, ctas_per_sm;
-    double eff;   // relative pair throughput of one SM running this variant (variant 0 = 1)
+    KernelShape s;
+    double eff;   // relative pair throughput of one SM running this shape (large = 1); measured, DESIGN.md "Plan"
 };
 
-// must match the template instantiations in force_f32.cu / force_f64.cu
 const VariantDesc kVariants[2][2] = {
-    /* PP_F32 */ {{256, 4, 256, 4, 2, 1.0}, {128, 1, 128, 4, 4, 0.45}},
-    /* PP_F64 */ {{256, 4, 256, 4, 1, 1.0}, {128, 1, 128, 4, 4, 0.80}},
+    /* PP_F32 */ {{kShapeF32Large, 1.0}, {kShapeF32Small, 0.45}},
+    /* PP_F64 */ {{kShapeF64Large, 1.0}, {kShapeF64Small, 0.80}},
 };
 
 int64_t round_up(int64_t a, int64_t b) { return (a + b - 1) / b * b; }
@@ -32,7 +31,8 @@ Plan make_plan(int64_t N, int precision, int sm_count, int64_t forced_split) {
     double best_cost = -1.0;
     const size_t elem = precision == PP_F64 ? 32 : 16;
     for (int v = 0; v < 2; ++v) {
-        const VariantDesc& d = kVariants[precision == PP_F64 ? 1 : 0][v];
+        const VariantDesc& vd = kVariants[precision == PP_F64 ? 1 : 0][v];
+        const KernelShape& d = vd.s;
         Plan p{};
         p.variant = v;
         p.threads = d.threads;
@@ -51,7 +51,7 @@ Plan make_plan(int64_t N, int precision, int sm_count, int64_t forced_split) {
                                           std::max<int64_t>(1, (int64_t)((1ull << 30) / (p.n_pad * elem))));
         int64_t s_lo = 1, s_hi = s_max;
         if (forced_split >= 1) s_lo = s_hi = std::min<int64_t>(forced_split, p.n_tiles);
-        const double tile_cost = (double)p.i_per_cta * p.tile_j * d.ctas_per_sm / d.eff;
+        const double tile_cost = (double)p.i_per_cta * p.tile_j * d.ctas_per_sm / vd.eff;
         for (int64_t S = s_lo; S <= s_hi; ++S) {
             const int64_t units = (int64_t)p.n_iblocks * S;
             const int64_t waves = (units + resident - 1) / resident;

@@ -19,11 +19,54 @@ void count_launch(int n = 1);
         if (e__ != cudaSuccess) return ::ppgrav::cuda_fail(e__, #call); \
     } while (0)
 
+// ---- kernel shapes: one table read by both the plan (plan.cu) and the instantiations (force_f32.cu/force_f64.cu) -------
+// "large" = the throughput shape used whenever it fills the machine, "small" = the fallback for tiny N.
+// Overridable at compile time (-DPP_F32_IPT=2 ...) for tuning sweeps; the defaults are the measured best.
+#ifndef PP_F32_THREADS
+#define PP_F32_THREADS 256
+#endif
+#ifndef PP_F32_IPT
+#define PP_F32_IPT 4
+#endif
+#ifndef PP_F32_TJ
+#define PP_F32_TJ 256
+#endif
+#ifndef PP_F32_MINB
+#define PP_F32_MINB 2
+#endif
+#ifndef PP_F32_UNROLL
+#define PP_F32_UNROLL 2
+#endif
+#ifndef PP_F64_THREADS
+#define PP_F64_THREADS 256
+#endif
+#ifndef PP_F64_IPT
+#define PP_F64_IPT 4
+#endif
+#ifndef PP_F64_TJ
+#define PP_F64_TJ 256
+#endif
+#ifndef PP_F64_MINB
+#define PP_F64_MINB 1
+#endif
+#ifndef PP_F64_UNROLL
+#define PP_F64_UNROLL 2
+#endif
+constexpr int kF32Unroll = PP_F32_UNROLL;   // j-pairs (FP32) / j-bodies (FP64) per unrolled loop body
+constexpr int kF64Unroll = PP_F64_UNROLL;
+struct KernelShape {
+    int threads, ipt, tile_j, stages, ctas_per_sm;
+};
+constexpr KernelShape kShapeF32Large = {PP_F32_THREADS, PP_F32_IPT, PP_F32_TJ, 4, PP_F32_MINB};
+constexpr KernelShape kShapeF32Small = {128, 1, 128, 4, 4};
+constexpr KernelShape kShapeF64Large = {PP_F64_THREADS, PP_F64_IPT, PP_F64_TJ, 4, PP_F64_MINB};
+constexpr KernelShape kShapeF64Small = {128, 1, 128, 4, 4};
+
 // ---- launch plan of one gravity solve (plan.cu) --------------------------------------------------------------
 // The all-pairs sweep is cut into work units (i-block, j-split): CTA (ib, s) sweeps the j-tiles of split s for the
 // bodies of i-block ib and writes one partial sum per body; a finalize kernel adds the S partials in fixed order.
 struct Plan {
-    int variant;        // 0 = large (256 threads x 4 i-bodies), 1 = small (128 threads x 1 i-body)
+    int variant;        // 0 = large shape, 1 = small shape (see KernelShape above)
     int threads;        // threads per CTA
     int ipt;            // i-bodies per thread
     int i_per_cta;      // threads * ipt

@@ -21,7 +21,7 @@ PP_CFG_SPLIT_J, PP_CFG_GRAPH, PP_CFG_PROFILE = 1, 2, 3
 INVARIANT_NAMES = ("E", "K", "W", "Px", "Py", "Pz", "Lx", "Ly", "Lz", "Cx", "Cy", "Cz", "M")
 PROBE_KINDS = {"ffma": 0, "ffma2": 1, "dfma": 2, "mufu_rsq": 3, "mufu_rsq64h": 4, "force_mix_f32": 5}
 
-LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libppgrav.so")
+LIB_PATH = os.environ.get("PPGRAV_LIB") or os.path.join(os.path.dirname(os.path.abspath(__file__)), "libppgrav.so")
 
 # every symbol include/ppgrav.h declares: (restype, argtypes)
 _i64, _dbl, _int, _vp, _u = ctypes.c_int64, ctypes.c_double, ctypes.c_int, ctypes.c_void_p, ctypes.c_uint
