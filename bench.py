@@ -128,34 +128,26 @@ def time_steps(torch, step_fn, steps, warmup, flush, barrier):
 def run_ours(args):
     import torch
     import torch.distributed as dist
-    from paper_1803_01190_b200 import ppgrav, workloads
+    from paper_1803_01190_b200 import ppgrav, replicas, workloads
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    rank, local, world = replicas.env_rank()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
-    def barrier():
-        if world > 1:
-            dist.barrier()
+    barrier = replicas.barrier
 
-    def max_over_ranks(x):
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)      # timing bookkeeping only: not on the data path
-        return float(t.item())
+    def max_over_ranks(x):                             # timing bookkeeping only: not on the data path
+        return replicas.max_over_ranks(x, device="cuda")
 
     ppgrav.lib()                                       # fails loudly if the CUDA library is missing
     c = workloads.config(args.config, N=args.n)
     c["index"] = args.config
     if world > 1:                                      # replicas: same recipe, a different seed per rank
         c = dict(c)
-        c["seed"] = c["seed"] + 1000 * rank
+        c["seed"] = replicas.replica_seed(c["seed"], rank)
         c["pos"], c["vel"], c["mass"] = workloads.make(c["kind"], c["N"], c["seed"], c.get("sigma_f", 0.1), c["G"])
     N, G, delta = c["N"], c["G"], c["delta"]
     dt = c["dt"] if c["dt"] > 0 else 2.5e-4
@@ -206,7 +198,7 @@ def run_ours(args):
         achieved = ops * pairs * sweep_n / (sweep_ms * 1e-3) / 1e12 if sweep_ms > 0 else 0.0
         inv = ppgrav.invariants_dict(out16)
         results[name] = dict(
-            value=world * pairs * args.steps / (ms * 1e-3), ms_per_step=ms / args.steps,
+            value=replicas.job_value(pairs, args.steps, ms, world), ms_per_step=ms / args.steps,
             sweep_ms_per_launch=sweep_ms / max(sweep_n, 1), sweep_share_of_step=sweep_ms / ms,
             roofline=dict(bound="alu", kernel="force_%s_kernel (pair sweep with potential)" % name,
                           achieved=achieved, peak=peak, unit="Tlane-op/s", frac=achieved / peak, traffic=None,
@@ -220,7 +212,7 @@ def run_ours(args):
             ppgrav.pp_forces(pos, mass, G=G, delta=delta, acc=acc)
 
         fms = max_over_ranks(time_steps(torch, force_only, max(2, args.steps // 2), 1, flush, barrier))
-        results[name]["force_only"] = world * pairs * max(2, args.steps // 2) / (fms * 1e-3)
+        results[name]["force_only"] = replicas.job_value(pairs, max(2, args.steps // 2), fms, world)
 
         if name == "f32" and not args.no_e2e:
             # end to end through the host-buffer C ABI: pinned host arrays in, results back, every step
@@ -244,7 +236,7 @@ def run_ours(args):
                 flush()
             torch.cuda.synchronize()
             ems = max_over_ranks((time.perf_counter() - t0) * 1e3)
-            results[name]["e2e"] = dict(value=world * pairs * args.steps / (ems * 1e-3), unit=UNIT,
+            results[name]["e2e"] = dict(value=replicas.job_value(pairs, args.steps, ems, world), unit=UNIT,
                                         h2d_bytes_per_step=int((10 * N + 8 * N) * el),
                                         d2h_bytes_per_step=int((10 * N) * el + 128),
                                         api="pp_step_kdk_host + pp_invariants_host (pinned host buffers)")

@@ -1,0 +1,190 @@
+"""GPU parity at BASELINE.json's full sizes (configs 1-4, N up to 2^23), in the launch configuration bench.py times.
+
+The oracle cannot sweep these sizes end to end (config 2's 100 steps are 1.1e14 pairs), so -- DESIGN.md section 6 --
+accelerations and potentials are compared on 4096 sampled bodies the oracle evaluates one by one, trajectories
+through oracle-evaluated invariants of the GPU's own snapshots, and a reduced-N run of the same recipe is compared
+with the oracle step for step.  Drift of E, P, L for FP32, FP64 and the oracle is written to
+gpurun_out/drift_r1.json when that folder exists (reported in BASELINE.md).
+"""
+import json
+import os
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+TOL = {"f64": 1e-12, "f32": 2e-5}
+_report = {}
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("a -m gpu test was started without a CUDA device")
+    from paper_1803_01190_b200 import ppgrav
+    ppgrav.lib()
+    yield ppgrav
+    out = os.path.join(ROOT, "gpurun_out")
+    if os.path.isdir(out) and _report:
+        with open(os.path.join(out, "drift_r1.json"), "w") as f:
+            json.dump(_report, f, indent=1, sort_keys=True)
+
+
+def _dtype(prec):
+    import torch
+    return torch.float64 if prec == "f64" else torch.float32
+
+
+def _seen(prec, a):
+    a = np.asarray(a, dtype=np.float64)
+    return a if prec == "f64" else a.astype(np.float32).astype(np.float64)
+
+
+def _dev(prec, a):
+    import torch
+    return torch.tensor(a, dtype=_dtype(prec), device="cuda")
+
+
+def _rel_rows(got, ref):
+    got = np.asarray(got, dtype=np.float64).reshape(len(ref), -1)
+    ref = np.asarray(ref, dtype=np.float64).reshape(len(ref), -1)
+    return np.linalg.norm(got - ref, axis=1) / np.linalg.norm(ref, axis=1)
+
+
+def _sampled_force_check(gpu, oracle, c, prec, want_pot, tag):
+    """pp_forces on the full system; acceleration (and potential) of 4096 sampled bodies against the oracle."""
+    from paper_1803_01190_b200 import workloads
+    pos, mass = _seen(prec, c["pos"]), _seen(prec, c["mass"])
+    idx = workloads.sample_indices(c["seed"], c["N"], 4096)
+    a_ref, p_ref = oracle.forces(pos, mass, G=c["G"], delta=c["delta"], idx=idx, want_pot=True, nthreads=0)
+    dpos, dmass = _dev(prec, pos), _dev(prec, mass)
+    acc, pot = gpu.pp_forces(dpos, dmass, G=c["G"], delta=c["delta"], want_pot=want_pot)
+    ea = _rel_rows(acc[idx].cpu().numpy(), a_ref)
+    rec = {"N": c["N"], "acc_err_max": float(ea.max()), "acc_err_median": float(np.median(ea)),
+           "acc_err_p999": float(np.quantile(ea, 0.999))}
+    assert ea.max() <= TOL[prec], rec
+    if want_pot:
+        ep = _rel_rows(pot[idx].cpu().numpy(), p_ref)
+        rec["pot_err_max"] = float(ep.max())
+        assert ep.max() <= TOL[prec], rec
+    _report["%s_%s" % (tag, prec)] = rec
+    return dpos, dmass, acc, pot
+
+
+def _drifts(series):
+    """series: list of invariants dicts over time -> (|dE|max/|E0|, |dP|max, |dLz|max/|Lz0|) per DESIGN.md R9."""
+    e0, p0, l0 = series[0]["E"], series[0]["P"], series[0]["L"][2]
+    de = max(abs(s["E"] - e0) for s in series) / abs(e0)
+    dp = max(float(np.linalg.norm(s["P"] - p0)) for s in series)
+    dl = max(abs(s["L"][2] - l0) for s in series) / abs(l0)
+    return {"dE_over_E0": de, "dP_abs": dp, "dLz_over_Lz0": dl}
+
+
+def _check_snapshot_invariants(gpu, oracle, prec, dpos, dvel, dmass, dpot, c, full_potential):
+    """pp_invariants of a GPU snapshot against the oracle's invariants of the same snapshot.  With full_potential the
+    oracle runs its own O(N^2) potential; otherwise it is handed the GPU's Phi (itself checked on sampled bodies)."""
+    pos, vel, mass = (t.cpu().numpy().astype(np.float64) for t in (dpos, dvel, dmass))
+    if full_potential:
+        got = gpu.invariants_dict(gpu.pp_invariants(dpos, dvel, dmass, G=c["G"], delta=c["delta"]))
+        ref = oracle.invariants(pos, vel, mass, G=c["G"], delta=c["delta"], nthreads=0)
+    else:
+        got = gpu.invariants_dict(gpu.pp_invariants(dpos, dvel, dmass, G=c["G"], delta=c["delta"], pot=dpot))
+        ref = oracle.invariants(pos, vel, mass, G=c["G"], delta=c["delta"], pot=dpot.cpu().numpy().astype(np.float64))
+    for k in ("E", "K", "W"):
+        assert abs(got[k] - ref[k]) <= 1e-12 * abs(ref[k]), (k, got[k], ref[k])
+    p_scale = float(np.sum(mass[:, None] * np.abs(vel)))
+    assert np.abs(got["P"] - ref["P"]).max() <= 1e-14 * p_scale
+    assert np.abs(got["L"] - ref["L"]).max() <= 1e-12 * np.abs(ref["L"]).max()
+    assert np.abs(got["COM"] - ref["COM"]).max() <= 1e-13
+    return got
+
+
+# ---- config 1: 2^16 disk + 2^16 halo, 200 KDK steps -----------------------------------------------------------------
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_config1_reduced_n_trajectory_against_oracle(gpu, oracle, prec):
+    """Same recipe, seed, dt and 200 steps at N = 4096 (2048 + 2048): the oracle integrates it fully."""
+    import torch
+    from paper_1803_01190_b200 import workloads
+    c = workloads.config(1, N=4096)
+    pos, vel, mass = (_seen(prec, c[k]) for k in ("pos", "vel", "mass"))
+    series = [oracle.invariants(pos, vel, mass, G=c["G"], delta=c["delta"], nthreads=0)]
+    p, v, a = pos, vel, None
+    for _ in range(4):                                   # 4 x 50 steps, invariants sampled in between
+        p, v, a, _ = oracle.kdk_halfkick(p, v, mass, c["dt"], 50, G=c["G"], delta=c["delta"], acc=a, nthreads=0)
+        series.append(oracle.invariants(p, v, mass, G=c["G"], delta=c["delta"], nthreads=0))
+    _report["config1_N4096_oracle"] = _drifts(series)
+    dpos, dvel, dmass = _dev(prec, pos), _dev(prec, vel), _dev(prec, mass)
+    dacc = torch.zeros_like(dpos)
+    gser = [gpu.invariants_dict(gpu.pp_invariants(dpos, dvel, dmass, G=c["G"], delta=c["delta"]))]
+    for k in range(4):
+        gpu.pp_step_kdk(dpos, dvel, dmass, dacc, c["dt"], 50, G=c["G"], delta=c["delta"], acc_valid=(k > 0))
+        gser.append(gpu.invariants_dict(gpu.pp_invariants(dpos, dvel, dmass, G=c["G"], delta=c["delta"])))
+    _report["config1_N4096_%s" % prec] = _drifts(gser)
+    tol = {"f64": 1e-10, "f32": 2e-5}[prec]             # 200 steps: rounding grows ~sqrt(steps), see DESIGN.md
+    assert np.abs(dpos.cpu().numpy() - p).max() / np.abs(p).max() <= tol
+    assert np.abs(dvel.cpu().numpy() - v).max() / np.abs(v).max() <= tol
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_config1_full_size(gpu, oracle, prec):
+    import torch
+    from paper_1803_01190_b200 import workloads
+    c = workloads.config(1)
+    dpos, dmass, dacc, _ = _sampled_force_check(gpu, oracle, c, prec, True, "config1_step0")
+    dvel = _dev(prec, _seen(prec, c["vel"]))
+    dpot = torch.empty_like(dmass)
+    series = [_check_snapshot_invariants(gpu, oracle, prec, dpos, dvel, dmass, None, c, full_potential=True)]
+    for k in range(4):
+        gpu.pp_step_kdk(dpos, dvel, dmass, dacc, c["dt"], c["nsteps"] // 4, G=c["G"], delta=c["delta"],
+                        acc_valid=True, pot=dpot)
+        series.append(gpu.invariants_dict(gpu.pp_invariants(dpos, dvel, dmass, G=c["G"], delta=c["delta"])))
+    # the final snapshot: the oracle recomputes everything, O(N^2) potential included (1.7e10 pairs)
+    last = _check_snapshot_invariants(gpu, oracle, prec, dpos, dvel, dmass, None, c, full_potential=True)
+    assert last["E"] == series[-1]["E"]
+    d = _drifts(series)
+    _report["config1_%s" % prec] = d
+    if prec == "f64":                                    # leapfrog conserves P and L exactly: FP64 sits at round-off
+        assert d["dP_abs"] <= 1e-13 and d["dLz_over_Lz0"] <= 1e-12 and d["dE_over_E0"] <= 1e-3
+    else:
+        assert d["dP_abs"] <= 1e-5 and d["dLz_over_Lz0"] <= 1e-5 and d["dE_over_E0"] <= 1e-3
+
+
+# ---- config 2: 2^20 disk, the bench workload -------------------------------------------------------------------------
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_config2_full_size_forces_and_100_steps(gpu, oracle, prec):
+    import torch
+    from paper_1803_01190_b200 import workloads
+    c = workloads.config(2)
+    dpos, dmass, dacc, dpot = _sampled_force_check(gpu, oracle, c, prec, True, "config2_step0")
+    dvel = _dev(prec, _seen(prec, c["vel"]))
+    inv0 = _check_snapshot_invariants(gpu, oracle, prec, dpos, dvel, dmass, dpot, c, full_potential=False)
+    gpu.pp_step_kdk(dpos, dvel, dmass, dacc, c["dt"], c["nsteps"], G=c["G"], delta=c["delta"], acc_valid=True,
+                    pot=dpot)
+    inv1 = _check_snapshot_invariants(gpu, oracle, prec, dpos, dvel, dmass, dpot, c, full_potential=False)
+    # acc and pot of the final snapshot on sampled bodies, recomputed by the oracle from the final positions
+    idx = workloads.sample_indices(c["seed"], c["N"], 4096)
+    pos1 = dpos.cpu().numpy().astype(np.float64)
+    a_ref, p_ref = oracle.forces(pos1, _seen(prec, c["mass"]), G=c["G"], delta=c["delta"], idx=idx, nthreads=0)
+    assert _rel_rows(dacc[idx].cpu().numpy(), a_ref).max() <= TOL[prec]
+    assert _rel_rows(dpot[idx].cpu().numpy(), p_ref).max() <= TOL[prec]
+    d = _drifts([inv0, inv1])
+    _report["config2_%s" % prec] = d
+    if prec == "f64":
+        assert d["dP_abs"] <= 1e-13 and d["dLz_over_Lz0"] <= 1e-12 and d["dE_over_E0"] <= 1e-3
+
+
+# ---- configs 3 and 4: one evaluation at 2^22 and 2^23 ------------------------------------------------------------------
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_config3_plummer_2p22(gpu, oracle, prec):
+    from paper_1803_01190_b200 import workloads
+    _sampled_force_check(gpu, oracle, workloads.config(3), prec, True, "config3")
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_config4_disk_halo_2p23(gpu, oracle, prec):
+    from paper_1803_01190_b200 import workloads
+    _sampled_force_check(gpu, oracle, workloads.config(4), prec, False, "config4")
+    gpu.pp_release()
