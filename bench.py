@@ -34,6 +34,9 @@ METRIC = "pair-interactions/s"
 UNIT = "pair-interactions/s"
 # nominal pipe peaks: lanes per SM x SMs x max SM clock
 FP32_LANES, FP64_LANES, SM_COUNT, SM_MAX_HZ = 128, 64, 148, 1.965e9
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE sweep launch (with potential) at N = 2^20, from the
+# `ncu --set full` captures summarised in profiles/r1_force_f32_ncu.md / profiles/r1_force_f64_ncu.md
+NCU_TRAFFIC_BYTES = {("f32", 1 << 20): 16.923136e6 + 0.117504e6, ("f64", 1 << 20): 34.294528e6 + 5.604352e6}
 L2_FLUSH_BYTES = 256 << 20
 
 
@@ -201,7 +204,8 @@ def run_ours(args):
             value=replicas.job_value(pairs, args.steps, ms, world), ms_per_step=ms / args.steps,
             sweep_ms_per_launch=sweep_ms / max(sweep_n, 1), sweep_share_of_step=sweep_ms / ms,
             roofline=dict(bound="alu", kernel="force_%s_kernel (pair sweep with potential)" % name,
-                          achieved=achieved, peak=peak, unit="Tlane-op/s", frac=achieved / peak, traffic=None,
+                          achieved=achieved, peak=peak, unit="Tlane-op/s", frac=achieved / peak,
+                          traffic=NCU_TRAFFIC_BYTES.get((name, N)),
                           pipe_ops_per_pair=ops,
                           peak_source="nominal: %d %s lanes/SM x %d SMs x %.0f MHz" %
                                       (lanes, "FP32" if name == "f32" else "FP64", SM_COUNT, SM_MAX_HZ / 1e6)),
