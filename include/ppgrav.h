@@ -118,8 +118,11 @@ int pp_invariants_host(const void* pos, const void* vel, const void* mass, const
 int pp_plan_query(int64_t N, int precision, int with_pot, int64_t* out8);
 
 /* Pipe-throughput microbenchmark used for the roofline denominators.
- *   kind: 0 FFMA, 1 FFMA2 (packed f32x2), 2 DFMA, 3 MUFU.RSQ, 4 MUFU.RSQ64H, 5 FFMA2+MUFU in the force kernel's mix (12 : 2)
- *   out4 (host) = { seconds, lane-operations executed, SM clock in MHz during the run, lane-ops/clk/SM }.
+ *   kind: 0 FFMA, 1 FFMA2 (packed f32x2), 2 DFMA, 3 MUFU.RSQ, 4 MUFU.RSQ64H, 5 FFMA2+MUFU in the force kernel's mix (12 : 2),
+ *         6 two FFMA2 : one DFMA with loop-constant multiplier/addend (do the FP32 and FP64 pipes overlap?),
+ *         7 FFMA2 with three distinct register operands, 8 as 6 with three distinct register operands each
+ *   out4 (host) = { seconds, lane-operations executed, SM clock in MHz during the run, lane-ops/clk/SM }; kinds 6-8
+ *   count the FFMA2 lanes only.
  * Synchronous. */
 int pp_probe_pipe(int kind, int64_t iters, double* out4);
 

@@ -26,13 +26,13 @@ void count_launch(int n = 1);
 #define PP_F32_THREADS 256
 #endif
 #ifndef PP_F32_IPT
-#define PP_F32_IPT 4
+#define PP_F32_IPT 6
 #endif
 #ifndef PP_F32_TJ
-#define PP_F32_TJ 256
+#define PP_F32_TJ 512
 #endif
 #ifndef PP_F32_MINB
-#define PP_F32_MINB 2
+#define PP_F32_MINB 1
 #endif
 #ifndef PP_F32_UNROLL
 #define PP_F32_UNROLL 2
@@ -41,7 +41,7 @@ void count_launch(int n = 1);
 #define PP_F64_THREADS 256
 #endif
 #ifndef PP_F64_IPT
-#define PP_F64_IPT 4
+#define PP_F64_IPT 6
 #endif
 #ifndef PP_F64_TJ
 #define PP_F64_TJ 256

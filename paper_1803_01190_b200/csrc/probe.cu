@@ -31,6 +31,10 @@ __device__ __forceinline__ double rsqrt_f64h(double x) {
 }
 
 // KIND: 0 FFMA, 1 FFMA2, 2 DFMA, 3 MUFU.RSQ, 4 MUFU.RSQ64H, 5 the force kernel's mix (12 FFMA2 : 2 MUFU.RSQ = two pairs)
+// 6-8 ask whether the idle FP64 pipe could carry extra i-bodies of an FP32 sweep:
+//   6 two FFMA2 : one DFMA, every instruction a = a*b + c with loop-constant b, c (one register operand read each)
+//   7 FFMA2 alone, three distinct rotating register operands per instruction (what a real pair loop reads)
+//   8 two FFMA2 : one DFMA, three distinct rotating register operands per instruction
 template <int KIND>
 __global__ void __launch_bounds__(kThreads, kCtasPerSm)
 probe_kernel(int64_t iters, float seed, float* __restrict__ sink, uint64_t* __restrict__ clk) {
@@ -96,6 +100,55 @@ probe_kernel(int64_t iters, float seed, float* __restrict__ sink, uint64_t* __re
                 for (int k = 0; k < kChains; ++k) a[k] = rsqrt_f64h(a[k]);
 #pragma unroll
         for (int k = 0; k < kChains; ++k) acc += (float)a[k];
+    } else if (KIND == 6) {
+        float2 a[kChains];
+        double d[kChains / 2];
+        const float tx = (seed + threadIdx.x) * 1e-9f;
+        const float2 b = make_float2(1.0f + tx, 1.0f - tx), c = make_float2(tx, seed + tx);
+        const double bd = 1.0 + tx, cd = tx;
+#pragma unroll
+        for (int k = 0; k < kChains; ++k) a[k] = make_float2(seed + k, seed + threadIdx.x);
+#pragma unroll
+        for (int k = 0; k < kChains / 2; ++k) d[k] = seed + k;
+        for (int64_t it = 0; it < iters; ++it)
+#pragma unroll
+            for (int u = 0; u < kInner; ++u)
+#pragma unroll
+                for (int k = 0; k < kChains / 2; ++k) {
+                    a[2 * k] = __ffma2_rn(a[2 * k], b, c);
+                    d[k] = __fma_rn(d[k], bd, cd);
+                    a[2 * k + 1] = __ffma2_rn(a[2 * k + 1], b, c);
+                }
+#pragma unroll
+        for (int k = 0; k < kChains; ++k) acc += a[k].x + a[k].y;
+#pragma unroll
+        for (int k = 0; k < kChains / 2; ++k) acc += (float)d[k];
+    } else if (KIND == 7 || KIND == 8) {
+        float2 a[kChains], x[kChains], y[kChains];
+        double d[kChains / 2], xd[kChains / 2], yd[kChains / 2];
+        const float tx = (seed + threadIdx.x) * 1e-9f;
+#pragma unroll
+        for (int k = 0; k < kChains; ++k) {
+            a[k] = make_float2(seed + k, seed + threadIdx.x);
+            x[k] = make_float2(1e-3f * k + tx, tx);
+            y[k] = make_float2(tx + k, 1.f + tx);
+        }
+#pragma unroll
+        for (int k = 0; k < kChains / 2; ++k) { d[k] = seed + k; xd[k] = 1e-3 * k + tx; yd[k] = tx + k; }
+        for (int64_t it = 0; it < iters; ++it)
+#pragma unroll
+            for (int u = 0; u < kInner; ++u)
+#pragma unroll
+                for (int k = 0; k < kChains / 2; ++k) {
+                    a[2 * k] = __ffma2_rn(x[(2 * k + u) % kChains], y[(2 * k + 3 + u) % kChains], a[2 * k]);
+                    if (KIND == 8)
+                        d[k] = __fma_rn(xd[(k + u) % (kChains / 2)], yd[(k + 1 + u) % (kChains / 2)], d[k]);
+                    a[2 * k + 1] = __ffma2_rn(x[(2 * k + 1 + u) % kChains], y[(2 * k + 4 + u) % kChains], a[2 * k + 1]);
+                }
+#pragma unroll
+        for (int k = 0; k < kChains; ++k) acc += a[k].x + a[k].y + x[k].x + y[k].y;
+#pragma unroll
+        for (int k = 0; k < kChains / 2; ++k) acc += (float)(d[k] + xd[k] + yd[k]);
     } else {
         float2 a[kChains];
         const float tx = (seed + threadIdx.x) * 1e-9f;
@@ -132,8 +185,8 @@ void launch(int grid, int64_t iters, float* sink, uint64_t* clk) {
 }  // namespace
 
 int run_probe(int kind, int64_t iters, int sm_count, double* out4) {
-    if (kind < 0 || kind > 5 || iters < 1) {
-        set_error("pp_probe_pipe: kind must be 0..5 and iters >= 1");
+    if (kind < 0 || kind > 8 || iters < 1) {
+        set_error("pp_probe_pipe: kind must be 0..8 and iters >= 1");
         return PP_EINVAL;
     }
     const int grid = sm_count * kCtasPerSm;
@@ -153,7 +206,10 @@ int run_probe(int kind, int64_t iters, int sm_count, double* out4) {
             case 2: launch<2>(grid, iters, sink, clk); break;
             case 3: launch<3>(grid, iters, sink, clk); break;
             case 4: launch<4>(grid, iters, sink, clk); break;
-            default: launch<5>(grid, iters, sink, clk); break;
+            case 5: launch<5>(grid, iters, sink, clk); break;
+            case 6: launch<6>(grid, iters, sink, clk); break;
+            case 7: launch<7>(grid, iters, sink, clk); break;
+            default: launch<8>(grid, iters, sink, clk); break;
         }
         count_launch();
         PP_CUDA(cudaGetLastError());
@@ -167,8 +223,9 @@ int run_probe(int kind, int64_t iters, int sm_count, double* out4) {
     cudaEventDestroy(e1);
     cudaFree(sink);
     cudaFree(clk);
-    // lane-operations per chain step: packed instructions count 2 lanes; the mix counts its 12 FFMA2 (24 lane-ops)
-    const double per_step = (kind == 1) ? 2.0 : (kind == 5) ? 24.0 : 1.0;
+    // lane-operations per chain step: packed instructions count 2 lanes; the mix counts its 12 FFMA2 (24 lane-ops);
+    // kinds 6-8 count their FFMA2 lanes only (kinds 6 and 8 also run one DFMA per two FFMA2 on the FP64 pipe)
+    const double per_step = (kind == 1 || kind >= 6) ? 2.0 : (kind == 5) ? 24.0 : 1.0;
     const double lane_ops = (double)grid * kThreads * (double)iters * kInner * kChains * per_step;
     const double sec = ms * 1e-3;
     const double mhz = h[1] ? (double)h[0] / (double)h[1] * 1e3 : 0.0;

@@ -19,7 +19,8 @@ PP_F32, PP_F64 = 0, 1
 PP_ACC_VALID = 1
 PP_CFG_SPLIT_J, PP_CFG_GRAPH, PP_CFG_PROFILE = 1, 2, 3
 INVARIANT_NAMES = ("E", "K", "W", "Px", "Py", "Pz", "Lx", "Ly", "Lz", "Cx", "Cy", "Cz", "M")
-PROBE_KINDS = {"ffma": 0, "ffma2": 1, "dfma": 2, "mufu_rsq": 3, "mufu_rsq64h": 4, "force_mix_f32": 5}
+PROBE_KINDS = {"ffma": 0, "ffma2": 1, "dfma": 2, "mufu_rsq": 3, "mufu_rsq64h": 4, "force_mix_f32": 5,
+               "ffma2_dfma_const": 6, "ffma2_3reg": 7, "ffma2_dfma_3reg": 8}
 
 LIB_PATH = os.environ.get("PPGRAV_LIB") or os.path.join(os.path.dirname(os.path.abspath(__file__)), "libppgrav.so")
 

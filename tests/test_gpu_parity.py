@@ -75,10 +75,10 @@ def test_forces_config0_all_bodies(gpu, oracle, prec):
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
-@pytest.mark.parametrize("n", [1, 2, 3, 127, 128, 129, 255, 257, 1000, 1023, 1025, 3001, 5000])
+@pytest.mark.parametrize("n", [1, 2, 3, 127, 128, 129, 255, 257, 511, 513, 1000, 1535, 1537, 3001, 5000])
 @pytest.mark.parametrize("split", [0, 1, 3])
 def test_forces_ragged_sizes_and_splits(gpu, oracle, prec, n, split):
-    """Sizes around the tile (128/256) and i-block (128/1024) edges, automatic and forced split-j, two mass species,
+    """Sizes around the tile (128/256/512) and i-block (128/1536) edges, automatic and forced split-j, two mass species,
     G != 1."""
     pos, _, mass = _random_cloud(n, 100 + n)
     pos, mass = _inputs_seen(prec, pos, mass)
