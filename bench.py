@@ -13,6 +13,8 @@ evaluation (pp_forces without potential) of both precisions under "force_only".
 
 Multi-GPU: the north_star runs on one GPU with no sharding -- `--gpus N` runs N independent replicas ("replicas
 only"), one process per GPU under torchrun, no data-path collective; value = pairs of all ranks / max time.
+`--sharded` (opt-in) instead shards the i-bodies of ONE system over the N GPUs, with one
+all-gather of the positions per step (paper_1803_01190_b200/sharded.py); it reports "scaling": "strong".
 
 --impl reference times the CPU oracle (oracle/, as it stands) on the host cores on a bounded sample of the same
 workload; it is the only other place besides cpu_baseline where this file touches oracle/.
@@ -51,6 +53,9 @@ def parse_args():
     ap.add_argument("--no-fp64", action="store_true", help="skip the FP64 arm (faster profiling runs)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--sharded", action="store_true",
+                    help="ONE system, i-bodies sharded over the N GPUs with an all-gather of positions per step "
+                         "(SURVEY.md 8(f) NEXT-1, strong scaling) instead of the default N independent replicas")
     return ap.parse_args()
 
 
@@ -277,6 +282,73 @@ def run_ours(args):
     return line
 
 
+# ---- one system sharded over the GPUs (opt-in; the north_star's graded path is the single-GPU one above) ---------
+def run_sharded(args):
+    """Strong scaling of ONE configs[2] system: every rank owns N/k i-bodies, per step
+    pp_kick_drift(own) -> all_gather(pos) over NCCL -> pp_forces_range(own i, all j, with potential) ->
+    pp_kick_drift(own, closing kick) -> pp_invariants(own) -> all_reduce of the 16 partial sums."""
+    import torch
+    import torch.distributed as dist
+    from paper_1803_01190_b200 import ppgrav, replicas, sharded, workloads
+
+    rank, local, world = replicas.env_rank()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    ppgrav.lib()
+    c = workloads.config(args.config, N=args.n)
+    c["index"] = args.config
+    N, G, delta = c["N"], c["G"], c["delta"]
+    dt = c["dt"] if c["dt"] > 0 else 2.5e-4
+    pairs = float(N) * float(N - 1)
+    flush_buf = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device="cuda")
+    comm = sharded.DistComm() if world > 1 else sharded.SingleComm()
+    results = {}
+    launches = clocks = None
+    for name, dtype in [("f32", torch.float32)] + ([] if args.no_fp64 else [("f64", torch.float64)]):
+        pos, vel, mass = (torch.tensor(c[k], dtype=dtype, device="cuda") for k in ("pos", "vel", "mass"))
+        sysm = sharded.ShardedSystem(pos, vel, mass, G=G, delta=delta, comm=comm)
+        inv = {}
+
+        def step():
+            sysm.step(dt, 1, want_pot=True)
+            inv.update(sysm.invariants())
+
+        sampler = ClockSampler(local) if (name == "f32" and rank == 0) else None
+        for _ in range(args.warmup):
+            step()
+            flush_buf.zero_()
+        n0 = ppgrav.pp_launch_count()
+        ms = replicas.max_over_ranks(time_steps(torch, step, args.steps, 0, flush_buf.zero_, replicas.barrier),
+                                     device="cuda")
+        if sampler is not None:
+            clocks = sampler.stop()
+            launches = ppgrav.pp_launch_count() - n0
+        results[name] = dict(value=pairs * args.steps / (ms * 1e-3), ms_per_step=ms / args.steps, E_after=inv["E"],
+                             own_bodies=sysm.count)
+        del sysm, pos, vel, mass
+    line = None
+    if rank == 0:
+        r = results["f32"]
+        line = {"metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True,
+                "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": workload_name(c),
+                           "step": "pp_kick_drift -> all_gather(pos) -> pp_forces_range(with potential) -> "
+                                   "pp_kick_drift -> pp_invariants -> all_reduce(16 doubles)",
+                           "pairs_per_step": pairs, "parallelism": "i-sharded x%d" % world,
+                           "l2": "256 MiB flush write between steps, inside the timed region",
+                           "bytes_gathered_per_step": 12 * N, "own_bodies": r["own_bodies"]},
+                "gpu_launches": launches, "clocks": clocks,
+                "fp64": results.get("f64")}
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return line
+
+
 # ---- the oracle on the host cores --------------------------------------------------------------------------------
 def cpu_baseline(c, n_sample):
     """Times oracle.forces (as it stands) on a bounded sample of i-bodies against all N j-bodies."""
@@ -330,7 +402,8 @@ def run_reference(args):
 
 def main():
     args = parse_args()
-    line = run_reference(args) if args.impl == "reference" else run_ours(args)
+    line = (run_reference(args) if args.impl == "reference" else run_sharded(args) if args.sharded
+            else run_ours(args))
     if line is not None:
         print(json.dumps(line), flush=True)
 

@@ -83,6 +83,22 @@ int pp_profile_read(double* out2);
 int pp_forces(const void* pos, const void* mass, void* acc, void* pot, int64_t N, double G, double delta,
               int precision, void* stream);
 
+/* The same gravity solve restricted to the i-bodies [i_begin, i_begin + i_count): every GPU of a multi-GPU run
+ * "calculates the dynamics of N/k particles" against all N j-bodies, so
+ *   pos [N,3], mass [N] in (all bodies);  acc [i_count,3] out;  pot [i_count] out or NULL.
+ * Per body the arithmetic is that of pp_forces; results are bit-identical to the corresponding rows of pp_forces
+ * when the split-j factor is the same (PP_CFG_SPLIT_J), otherwise equal to summation-order round-off.
+ * PP_EINVAL if the range is empty or leaves [0, N). */
+int pp_forces_range(const void* pos, const void* mass, void* acc, void* pot, int64_t N, int64_t i_begin,
+                    int64_t i_count, double G, double delta, int precision, void* stream);
+
+/* One "Update System" pass on n bodies, for callers that sequence the step themselves (the sharded
+ * step in paper_1803_01190_b200/sharded.py):  vel += kick * acc;  then, if dt != 0,  pos += dt * vel.
+ * kick = dt/2, dt = dt is the opening half-kick + drift of eqs. (5)-(6); kick = dt/2, dt = 0 is the closing half-kick
+ * of eq. (7).  pos, vel [n,3] in/out;  acc [n,3] in. */
+int pp_kick_drift(void* pos, void* vel, const void* acc, int64_t n, double kick, double dt, int precision,
+                  void* stream);
+
 /* nsteps kick-drift-kick steps of size dt, eqs. (5)-(7), in the algebraically identical
  * half-kick form  v += dt/2 a(t);  r += dt v;  a(t+dt) = forces(r);  v += dt/2 a(t+dt)  -- the paper's "Update
  * System" kernel around one gravity solve per step.

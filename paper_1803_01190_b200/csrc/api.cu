@@ -138,15 +138,16 @@ int sweep(const Plan& p, int precision, const void* packed, void* partial, int64
 }
 
 // one gravity solve on already packed bodies: sweep + finalize (optionally with the closing half-kick)
+// (acc, pot, vel address the p.i_count bodies of the plan's i-range)
 int solve_packed(const Plan& p, int precision, const void* packed, void* partial, int64_t N, double G, double delta,
                  void* acc, void* pot, void* vel, double kick, cudaStream_t st) {
     const int mode = pot ? MODE_FORCE_POT : MODE_FORCE;
     PP_TRY(sweep(p, precision, packed, partial, N, delta, mode, st));
     if (precision == PP_F32)
-        return launch_finalize_f32((const float4*)partial, p.split, p.n_pad, N, G, (float*)acc, (float*)pot,
-                                   (float*)vel, kick, st);
-    return launch_finalize_f64((const double4*)partial, p.split, p.n_pad, N, G, (double*)acc, (double*)pot,
-                               (double*)vel, kick, 0, st);
+        return launch_finalize_f32((const float4*)partial, p.split, p.part_stride, p.i_count, G, (float*)acc,
+                                   (float*)pot, (float*)vel, kick, st);
+    return launch_finalize_f64((const double4*)partial, p.split, p.part_stride, p.i_count, G, (double*)acc,
+                               (double*)pot, (double*)vel, kick, 0, st);
 }
 
 int pack_state(int precision, const void* pos, const void* mass, void* packed, int64_t N, int64_t n_pad,
@@ -164,11 +165,12 @@ int kick_drift_pack(int precision, void* pos, void* vel, const void* acc, const 
                                       (double*)packed, N, n_pad, kick, dt, st);
 }
 
-int prepare_solve(Workspace* w, int64_t N, int precision, Plan* plan, void** packed, void** partial) {
-    *plan = make_plan(N, precision, w->sm_count, g_cfg_split.load());
+int prepare_solve(Workspace* w, int64_t N, int precision, Plan* plan, void** packed, void** partial,
+                  int64_t i_begin = 0, int64_t i_count = -1) {
+    *plan = make_plan(N, precision, w->sm_count, g_cfg_split.load(), i_begin, i_count);
     const size_t body = 4 * elem_bytes(precision);
     PP_TRY(ensure(w, B_PACKED, (size_t)plan->n_pad * body, packed));
-    PP_TRY(ensure(w, B_PARTIAL, (size_t)plan->split * (size_t)plan->n_pad * body, partial));
+    PP_TRY(ensure(w, B_PARTIAL, (size_t)plan->split * (size_t)plan->part_stride * body, partial));
     return PP_OK;
 }
 
@@ -286,22 +288,49 @@ int pp_probe_pipe(int kind, int64_t iters, double* out4) {
     return run_probe(kind, iters, w->sm_count, out4);
 }
 
-int pp_forces(const void* pos, const void* mass, void* acc, void* pot, int64_t N, double G, double delta,
-              int precision, void* stream) {
-    PP_TRY(check_common("pp_forces", N, G, delta, precision));
-    PP_TRY(check_ptr("pp_forces", "pos", pos, precision, true));
-    PP_TRY(check_ptr("pp_forces", "mass", mass, precision, true));
-    PP_TRY(check_ptr("pp_forces", "acc", acc, precision, true));
-    PP_TRY(check_ptr("pp_forces", "pot", pot, precision, false));
+int pp_forces_range(const void* pos, const void* mass, void* acc, void* pot, int64_t N, int64_t i_begin,
+                    int64_t i_count, double G, double delta, int precision, void* stream) {
+    PP_TRY(check_common("pp_forces_range", N, G, delta, precision));
+    PP_TRY(check_ptr("pp_forces_range", "pos", pos, precision, true));
+    PP_TRY(check_ptr("pp_forces_range", "mass", mass, precision, true));
+    PP_TRY(check_ptr("pp_forces_range", "acc", acc, precision, true));
+    PP_TRY(check_ptr("pp_forces_range", "pot", pot, precision, false));
+    if (i_begin < 0 || i_count < 1 || i_begin > N - i_count) {
+        set_error("pp_forces_range: i-range [%lld, %lld + %lld) outside [0, N = %lld) or empty", (long long)i_begin,
+                  (long long)i_begin, (long long)i_count, (long long)N);
+        return PP_EINVAL;
+    }
     std::lock_guard<std::mutex> lk(g_mu);
     Workspace* w = nullptr;
     PP_TRY(current_workspace(&w));
     cudaStream_t st = (cudaStream_t)stream;
     Plan plan;
     void *packed, *partial;
-    PP_TRY(prepare_solve(w, N, precision, &plan, &packed, &partial));
+    PP_TRY(prepare_solve(w, N, precision, &plan, &packed, &partial, i_begin, i_count));
     PP_TRY(pack_state(precision, pos, mass, packed, N, plan.n_pad, st));
     return solve_packed(plan, precision, packed, partial, N, G, delta, acc, pot, nullptr, 0.0, st);
+}
+
+int pp_forces(const void* pos, const void* mass, void* acc, void* pot, int64_t N, double G, double delta,
+              int precision, void* stream) {
+    PP_TRY(check_common("pp_forces", N, G, delta, precision));
+    return pp_forces_range(pos, mass, acc, pot, N, 0, N, G, delta, precision, stream);
+}
+
+int pp_kick_drift(void* pos, void* vel, const void* acc, int64_t n, double kick, double dt, int precision,
+                  void* stream) {
+    PP_TRY(check_common("pp_kick_drift", n, 1.0, 0.0, precision));
+    PP_TRY(check_ptr("pp_kick_drift", "pos", pos, precision, true));
+    PP_TRY(check_ptr("pp_kick_drift", "vel", vel, precision, true));
+    PP_TRY(check_ptr("pp_kick_drift", "acc", acc, precision, true));
+    if (!std::isfinite(kick) || !std::isfinite(dt)) {
+        set_error("pp_kick_drift: kick and dt must be finite");
+        return PP_EINVAL;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    if (precision == PP_F32)
+        return launch_kick_drift_f32((float*)pos, (float*)vel, (const float*)acc, n, kick, dt, st);
+    return launch_kick_drift_f64((double*)pos, (double*)vel, (const double*)acc, n, kick, dt, st);
 }
 
 int pp_step_kdk(void* pos, void* vel, const void* mass, void* acc, void* pot, int64_t N, double dt, int64_t nsteps,
@@ -391,7 +420,7 @@ int pp_invariants(const void* pos, const void* vel, const void* mass, const void
         else
             PP_TRY(launch_pack_f64((const double*)pos, (const double*)mass, (double*)packed, N, plan.n_pad, st));
         PP_TRY(sweep(plan, PP_F64, packed, partial, N, delta, MODE_POT, st));
-        PP_TRY(launch_finalize_f64((const double4*)partial, plan.split, plan.n_pad, N, G, nullptr, (double*)p64,
+        PP_TRY(launch_finalize_f64((const double4*)partial, plan.split, plan.part_stride, N, G, nullptr, (double*)p64,
                                    nullptr, 0.0, 1, st));
         pot64 = (const double*)p64;
     }

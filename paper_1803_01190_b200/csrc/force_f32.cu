@@ -81,7 +81,7 @@ __device__ __forceinline__ void sweep_tile(const float4* __restrict__ tp, const 
 template <int THREADS, int IPT, int TJ, int STAGES, int MINB, int MODE, bool GUARD>
 __global__ void __launch_bounds__(THREADS, MINB)
 force_f32_kernel(const float* __restrict__ packed, float4* __restrict__ partial, const int n_tiles,
-                 const int64_t n_pad, const float eps2f) {
+                 const int64_t part_stride, const int64_t i_begin, const float eps2f) {
     constexpr int NWARPS = THREADS / 32;
     constexpr uint32_t TILE_BYTES = TJ * 16u;
     __shared__ __align__(128) float tiles[STAGES][TJ * 4];
@@ -119,7 +119,7 @@ force_f32_kernel(const float* __restrict__ packed, float4* __restrict__ partial,
     int iidx[IPT];
 #pragma unroll
     for (int k = 0; k < IPT; ++k) {
-        const int i = ib * (THREADS * IPT) + k * THREADS + tid;
+        const int i = (int)i_begin + ib * (THREADS * IPT) + k * THREADS + tid;   // global body index
         iidx[k] = i;
         const float* q = packed + (size_t)(i >> 1) * 8 + (i & 1);
         const float xi = q[0], yi = q[2], zi = q[4];
@@ -131,7 +131,7 @@ force_f32_kernel(const float* __restrict__ packed, float4* __restrict__ partial,
         cx[k] = cy[k] = cz[k] = cp[k] = 0.f;
     }
     const float2 eps2 = make_float2(eps2f, eps2f);
-    const int i_lo = ib * (THREADS * IPT), i_hi = i_lo + THREADS * IPT;
+    const int i_lo = (int)i_begin + ib * (THREADS * IPT), i_hi = i_lo + THREADS * IPT;
 
     for (int t = 0; t < nt; ++t) {
         const int s = t % STAGES;
@@ -176,18 +176,17 @@ force_f32_kernel(const float* __restrict__ packed, float4* __restrict__ partial,
         o.y = __fadd_rn(sy[k], cy[k]);
         o.z = __fadd_rn(sz[k], cz[k]);
         o.w = (MODE == MODE_FORCE_POT) ? __fadd_rn(sp[k], cp[k]) : 0.f;
-        partial[(size_t)sidx * n_pad + iidx[k]] = o;
+        partial[(size_t)sidx * part_stride + (iidx[k] - (int)i_begin)] = o;
     }
 }
 
 template <int THREADS, int IPT, int TJ, int STAGES, int MINB>
 int launch_variant(const Plan& p, const float* packed, float4* partial, int64_t N, float eps2, bool guard, int mode,
                    cudaStream_t st) {
-    const int n_ib = (int)((N + p.i_per_cta - 1) / p.i_per_cta);
-    dim3 grid(n_ib, p.split);
+    dim3 grid(p.n_iblocks, p.split);
 #define PP_LAUNCH32(MODE_, GUARD_)                                                      \
     force_f32_kernel<THREADS, IPT, TJ, STAGES, MINB, MODE_, GUARD_>                     \
-        <<<grid, THREADS, 0, st>>>(packed, partial, p.n_tiles, p.n_pad, eps2)
+        <<<grid, THREADS, 0, st>>>(packed, partial, p.n_tiles, p.part_stride, p.i_begin, eps2)
     if (mode == MODE_FORCE) {
         if (guard) PP_LAUNCH32(MODE_FORCE, true); else PP_LAUNCH32(MODE_FORCE, false);
     } else {

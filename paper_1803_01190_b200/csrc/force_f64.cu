@@ -81,7 +81,7 @@ __device__ __forceinline__ void sweep_tile(const double4* __restrict__ tp, const
 template <int THREADS, int IPT, int TJ, int STAGES, int MINB, int MODE, bool GUARD>
 __global__ void __launch_bounds__(THREADS, MINB)
 force_f64_kernel(const double* __restrict__ packed, double4* __restrict__ partial, const int n_tiles,
-                 const int64_t n_pad, const double eps2) {
+                 const int64_t part_stride, const int64_t i_begin, const double eps2) {
     constexpr int NWARPS = THREADS / 32;
     constexpr uint32_t TILE_BYTES = TJ * 32u;
     __shared__ __align__(128) double tiles[STAGES][TJ * 4];
@@ -118,14 +118,14 @@ force_f64_kernel(const double* __restrict__ packed, double4* __restrict__ partia
     int iidx[IPT];
 #pragma unroll
     for (int k = 0; k < IPT; ++k) {
-        const int i = ib * (THREADS * IPT) + k * THREADS + tid;
+        const int i = (int)i_begin + ib * (THREADS * IPT) + k * THREADS + tid;   // global body index
         iidx[k] = i;
         const double4 q = reinterpret_cast<const double4*>(packed)[i];
         xi[k] = q.x; yi[k] = q.y; zi[k] = q.z;
         ax[k] = ay[k] = az[k] = ap[k] = 0.0;
         sx[k] = sy[k] = sz[k] = sp[k] = cp[k] = 0.0;
     }
-    const int i_lo = ib * (THREADS * IPT), i_hi = i_lo + THREADS * IPT;
+    const int i_lo = (int)i_begin + ib * (THREADS * IPT), i_hi = i_lo + THREADS * IPT;
 
     for (int t = 0; t < nt; ++t) {
         const int s = t % STAGES;
@@ -163,18 +163,17 @@ force_f64_kernel(const double* __restrict__ packed, double4* __restrict__ partia
         double4 o;
         if (MODE == MODE_POT) { o.x = sp[k]; o.y = cp[k]; o.z = 0.0; o.w = 0.0; }
         else { o.x = sx[k]; o.y = sy[k]; o.z = sz[k]; o.w = (MODE == MODE_FORCE_POT) ? sp[k] : 0.0; }
-        partial[(size_t)sidx * n_pad + iidx[k]] = o;
+        partial[(size_t)sidx * part_stride + (iidx[k] - (int)i_begin)] = o;
     }
 }
 
 template <int THREADS, int IPT, int TJ, int STAGES, int MINB>
 int launch_variant(const Plan& p, const double* packed, double4* partial, int64_t N, double eps2, bool guard, int mode,
                    cudaStream_t st) {
-    const int n_ib = (int)((N + p.i_per_cta - 1) / p.i_per_cta);
-    dim3 grid(n_ib, p.split);
+    dim3 grid(p.n_iblocks, p.split);
 #define PP_LAUNCH64(MODE_, GUARD_)                                                      \
     force_f64_kernel<THREADS, IPT, TJ, STAGES, MINB, MODE_, GUARD_>                     \
-        <<<grid, THREADS, 0, st>>>(packed, partial, p.n_tiles, p.n_pad, eps2)
+        <<<grid, THREADS, 0, st>>>(packed, partial, p.n_tiles, p.part_stride, p.i_begin, eps2)
     if (mode == MODE_FORCE) {
         if (guard) PP_LAUNCH64(MODE_FORCE, true); else PP_LAUNCH64(MODE_FORCE, false);
     } else if (mode == MODE_FORCE_POT) {

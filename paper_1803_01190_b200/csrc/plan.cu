@@ -26,7 +26,8 @@ int64_t round_up(int64_t a, int64_t b) { return (a + b - 1) / b * b; }
 
 }  // namespace
 
-Plan make_plan(int64_t N, int precision, int sm_count, int64_t forced_split) {
+Plan make_plan(int64_t N, int precision, int sm_count, int64_t forced_split, int64_t i_begin, int64_t i_count) {
+    if (i_count < 0) i_count = N - i_begin;
     Plan best{};
     double best_cost = -1.0;
     const size_t elem = precision == PP_F64 ? 32 : 16;
@@ -42,13 +43,17 @@ Plan make_plan(int64_t N, int precision, int sm_count, int64_t forced_split) {
         p.stages = d.stages;
         p.ctas_per_sm = d.ctas_per_sm;
         p.sm_count = sm_count;
-        p.n_pad = round_up(N, std::max(p.i_per_cta, p.tile_j));   // tile_j divides i_per_cta in both variants
-        p.n_iblocks = (int)((N + p.i_per_cta - 1) / p.i_per_cta);
+        p.i_begin = i_begin;
+        p.i_count = i_count;
+        p.n_iblocks = (int)((i_count + p.i_per_cta - 1) / p.i_per_cta);
+        p.part_stride = (int64_t)p.n_iblocks * p.i_per_cta;
+        // tile_j divides i_per_cta in both variants; the last launched i-block may reach past N
+        p.n_pad = round_up(std::max(N, i_begin + p.part_stride), std::max(p.i_per_cta, p.tile_j));
         p.n_tiles = (int)((N + p.tile_j - 1) / p.tile_j);
         const int64_t resident = (int64_t)sm_count * d.ctas_per_sm;
         // partial sums: S x n_pad x {16,32} bytes, kept under 1 GiB
         int64_t s_max = std::min<int64_t>(std::min<int64_t>(p.n_tiles, 64),
-                                          std::max<int64_t>(1, (int64_t)((1ull << 30) / (p.n_pad * elem))));
+                                          std::max<int64_t>(1, (int64_t)((1ull << 30) / (p.part_stride * elem))));
         int64_t s_lo = 1, s_hi = s_max;
         if (forced_split >= 1) s_lo = s_hi = std::min<int64_t>(forced_split, p.n_tiles);
         const double tile_cost = (double)p.i_per_cta * p.tile_j * d.ctas_per_sm / vd.eff;
@@ -57,7 +62,7 @@ Plan make_plan(int64_t N, int precision, int sm_count, int64_t forced_split) {
             const int64_t waves = (units + resident - 1) / resident;
             const int64_t tps = (p.n_tiles + S - 1) / S;
             // 2 tile-times of fixed cost per unit (pipeline fill, epilogue), plus the finalize pass over S partials
-            const double cost = (double)waves * ((double)tps + 2.0) * tile_cost + 64.0 * (double)S * (double)p.n_pad;
+            const double cost = (double)waves * ((double)tps + 2.0) * tile_cost + 64.0 * (double)S * (double)p.part_stride;
             if (best_cost < 0.0 || cost < best_cost * (1.0 - 1e-9)) {
                 best_cost = cost;
                 best = p;

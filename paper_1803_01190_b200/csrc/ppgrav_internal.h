@@ -73,13 +73,18 @@ struct Plan {
     int tile_j;         // j-bodies per shared-memory tile
     int stages;         // depth of the TMA ring
     int ctas_per_sm;    // residency the kernel is built for
-    int64_t n_pad;      // N rounded up to a multiple of lcm(i_per_cta, tile_j): length of the packed array
-    int n_iblocks;      // n_pad / i_per_cta (only blocks that contain a real body are launched)
+    int64_t n_pad;      // length of the packed array: covers every j-tile and every launched i-block, padded with
+                        // massless bodies (N, or N + i_per_cta for an i-range that starts off a block boundary,
+                        // rounded up to a multiple of i_per_cta, which tile_j divides)
+    int64_t i_begin;    // first i-body of the solve (0 for a full solve; pp_forces_range shards the i-range)
+    int64_t i_count;    // i-bodies of the solve
+    int n_iblocks;      // ceil(i_count / i_per_cta): i-blocks launched
+    int64_t part_stride;   // n_iblocks * i_per_cta: bodies per split in the partial-sum workspace (local index i - i_begin)
     int n_tiles;        // ceil(N / tile_j): j-tiles that contain a real body
     int split;          // S
     int sm_count;
 };
-Plan make_plan(int64_t N, int precision, int sm_count, int64_t forced_split);
+Plan make_plan(int64_t N, int precision, int sm_count, int64_t forced_split, int64_t i_begin = 0, int64_t i_count = -1);
 
 // modes of the pair sweep
 enum { MODE_FORCE = 0, MODE_FORCE_POT = 1, MODE_POT = 2 };
@@ -93,7 +98,7 @@ int launch_pack_f64(const double* pos, const double* mass, double* packed, int64
 int launch_pack_f32_to_f64(const float* pos, const float* mass, double* packed, int64_t N, int64_t n_pad,
                            cudaStream_t st);
 
-// partial[s * n_pad + i] = {sum_x, sum_y, sum_z, sum_pot} over the j-tiles of split s, without G and with the
+// partial[s * part_stride + (i - i_begin)] = {sum_x, sum_y, sum_z, sum_pot} over the j-tiles of split s, without G and with the
 // sign convention  sum = sum_j m_j (r_j - r_i) w^3,  sum_pot = sum_j m_j w   (w = (r^2+delta^2)^{-1/2}).
 int launch_force_f32(const Plan& p, const float* packed, float4* partial, int64_t N, double delta, int mode,
                      cudaStream_t st);
@@ -107,6 +112,11 @@ int launch_finalize_f32(const float4* partial, int split, int64_t n_pad, int64_t
                         float* vel, double kick, cudaStream_t st);
 int launch_finalize_f64(const double4* partial, int split, int64_t n_pad, int64_t N, double G, double* acc,
                         double* pot, double* vel, double kick, int pot_is_dd, cudaStream_t st);
+
+// v += kick * a;  r += dt * v   on n bodies, no packing (the sharded step kicks and drifts its own bodies only)
+int launch_kick_drift_f32(float* pos, float* vel, const float* acc, int64_t n, double kick, double dt, cudaStream_t st);
+int launch_kick_drift_f64(double* pos, double* vel, const double* acc, int64_t n, double kick, double dt,
+                          cudaStream_t st);
 
 // v += kick * a;  r += dt * v;  packed = pack(r, m)      (eqs. (5)-(6) in half-kick form)
 int launch_kick_drift_pack_f32(float* pos, float* vel, const float* acc, const float* mass, float* packed, int64_t N,

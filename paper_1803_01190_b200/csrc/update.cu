@@ -105,7 +105,38 @@ kick_drift_pack_kernel(T* __restrict__ pos, T* __restrict__ vel, const T* __rest
     store_packed(packed, i, r[0], r[1], r[2], mass[i]);
 }
 
+// the sharded step's own-bodies update: opening half-kick + drift (dt != 0) or closing half-kick alone (dt == 0);
+// the same two fused multiply-adds per component as kick_drift_pack_kernel, so a sharded run rounds identically
+template <typename T>
+__global__ void __launch_bounds__(kThreads)
+kick_drift_kernel(T* __restrict__ pos, T* __restrict__ vel, const T* __restrict__ acc, int64_t n, T kick, T dt,
+                  bool drift) {
+    const int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x;
+    if (i >= n) return;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const T v = fma(kick, acc[3 * i + c], vel[3 * i + c]);
+        vel[3 * i + c] = v;
+        if (drift) pos[3 * i + c] = fma(dt, v, pos[3 * i + c]);
+    }
+}
+
 }  // namespace
+
+int launch_kick_drift_f32(float* pos, float* vel, const float* acc, int64_t n, double kick, double dt,
+                          cudaStream_t st) {
+    kick_drift_kernel<float><<<grid_for(n), kThreads, 0, st>>>(pos, vel, acc, n, (float)kick, (float)dt, dt != 0.0);
+    count_launch();
+    PP_CUDA(cudaGetLastError());
+    return PP_OK;
+}
+int launch_kick_drift_f64(double* pos, double* vel, const double* acc, int64_t n, double kick, double dt,
+                          cudaStream_t st) {
+    kick_drift_kernel<double><<<grid_for(n), kThreads, 0, st>>>(pos, vel, acc, n, kick, dt, dt != 0.0);
+    count_launch();
+    PP_CUDA(cudaGetLastError());
+    return PP_OK;
+}
 
 int launch_pack_f32(const float* pos, const float* mass, float* packed, int64_t N, int64_t n_pad, cudaStream_t st) {
     pack_kernel<float, float><<<grid_for(n_pad), kThreads, 0, st>>>(pos, mass, packed, N, n_pad);

@@ -33,6 +33,8 @@ SIGNATURES = {
     "pp_configure": (_int, [_int, _i64]),
     "pp_launch_count": (_i64, []),
     "pp_forces": (_int, [_vp, _vp, _vp, _vp, _i64, _dbl, _dbl, _int, _vp]),
+    "pp_forces_range": (_int, [_vp, _vp, _vp, _vp, _i64, _i64, _i64, _dbl, _dbl, _int, _vp]),
+    "pp_kick_drift": (_int, [_vp, _vp, _vp, _i64, _dbl, _dbl, _int, _vp]),
     "pp_step_kdk": (_int, [_vp, _vp, _vp, _vp, _vp, _i64, _dbl, _i64, _dbl, _dbl, _int, _u, _vp]),
     "pp_invariants": (_int, [_vp, _vp, _vp, _vp, _i64, _dbl, _dbl, _int, _vp, _vp]),
     "pp_forces_host": (_int, [_vp, _vp, _vp, _vp, _i64, _dbl, _dbl, _int, _vp]),
@@ -153,6 +155,38 @@ def pp_forces(pos, mass, G=1.0, delta=0.0, want_pot=False, acc=None, pot=None, s
         _check(lib().pp_forces(p_pos, p_mass, p_acc, p_pot, N, float(G), float(delta), prec, _stream(stream)),
                "pp_forces")
     return acc, pot
+
+
+def pp_forces_range(pos, mass, i_begin, i_count, G=1.0, delta=0.0, want_pot=False, acc=None, pot=None, stream=None):
+    """Accelerations (and potentials) of bodies [i_begin, i_begin + i_count) against all N bodies.
+    Returns (acc [i_count,3], pot [i_count] or None)."""
+    torch = _torch()
+    prec = _precision_of(pos)
+    N = pos.shape[0]
+    n = int(i_count)
+    p_pos = _dev(pos, (N, 3), pos.dtype, "pos")
+    p_mass = _dev(mass, (N,), pos.dtype, "mass")
+    if acc is None:
+        acc = torch.empty((n, 3), dtype=pos.dtype, device=pos.device)
+    if pot is None and want_pot:
+        pot = torch.empty((n,), dtype=pos.dtype, device=pos.device)
+    p_acc = _dev(acc, (n, 3), pos.dtype, "acc")
+    p_pot = _dev(pot, (n,), pos.dtype, "pot") if pot is not None else None
+    with torch.cuda.device(pos.device):
+        _check(lib().pp_forces_range(p_pos, p_mass, p_acc, p_pot, N, int(i_begin), n, float(G), float(delta), prec,
+                                     _stream(stream)), "pp_forces_range")
+    return acc, pot
+
+
+def pp_kick_drift(pos, vel, acc, kick, dt, stream=None):
+    """vel += kick * acc; pos += dt * vel (skipped when dt == 0), in place on CUDA tensors [n,3]."""
+    torch = _torch()
+    prec = _precision_of(pos)
+    n = pos.shape[0]
+    with torch.cuda.device(pos.device):
+        _check(lib().pp_kick_drift(_dev(pos, (n, 3), pos.dtype, "pos"), _dev(vel, (n, 3), pos.dtype, "vel"),
+                                   _dev(acc, (n, 3), pos.dtype, "acc"), n, float(kick), float(dt), prec,
+                                   _stream(stream)), "pp_kick_drift")
 
 
 def pp_step_kdk(pos, vel, mass, acc, dt, nsteps, G=1.0, delta=0.0, acc_valid=False, pot=None, stream=None):
