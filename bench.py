@@ -38,7 +38,7 @@ UNIT = "pair-interactions/s"
 FP32_LANES, FP64_LANES, SM_COUNT, SM_MAX_HZ = 128, 64, 148, 1.965e9
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE sweep launch (with potential) at N = 2^20, from the
 # `ncu --set full` captures summarised in profiles/r1_force_f32_ncu.md / profiles/r1_force_f64_ncu.md
-NCU_TRAFFIC_BYTES = {("f32", 1 << 20): 16.923136e6 + 0.117504e6, ("f64", 1 << 20): 34.294528e6 + 5.604352e6}
+NCU_TRAFFIC_BYTES = {("f32", 1 << 20): 17.068288e6 + 3.349760e6, ("f64", 1 << 20): 43.715584e6 + 57.617664e6}
 L2_FLUSH_BYTES = 256 << 20
 
 

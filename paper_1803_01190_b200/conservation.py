@@ -1,0 +1,93 @@
+"""Long-run conservation experiment: the paper's Table 2 / Figs. 5-6 on the built path.
+
+PAPER.md:146-176: for N = 128k ... 1024k the authors integrate an equilibrium stellar disk for 10^4 steps in single and
+in double precision and record max |dP|, max |dL|/L0, max |dE|/E0 (Table 2) and their time series
+(Figs. 5-6).  Their initial conditions cannot be regenerated, so this runs the same protocol on
+the synthetic Toomre-unstable exponential disk of BASELINE.json configs[2] (same recipe and seed, any N):
+
+    python -m paper_1803_01190_b200.conservation --logn 17 --steps 10000 --sample-every 100 --out gpurun_out/x.json
+
+Everything runs through the library: pp_step_kdk advances `sample_every` steps per call, pp_invariants evaluates
+E, P, L, COM of the snapshot with its own O(N^2) FP64 potential pass on the (promoted) state, so the diagnostic is
+equally accurate for both state precisions (reading R7) and FP32 drift is not masked by an FP32 potential.
+Drift definitions: DESIGN.md reading R9.
+"""
+import argparse
+import json
+import time
+
+import numpy as np
+
+
+def run(logn, steps, dt, sample_every, precision, config_index=2, verbose=True):
+    import torch
+    from . import ppgrav, workloads
+
+    N = 1 << logn
+    c = workloads.config(config_index, N=N)
+    G, delta = c["G"], c["delta"]
+    dtype = torch.float32 if precision == "f32" else torch.float64
+    pos, vel, mass = (torch.tensor(c[k], dtype=dtype, device="cuda") for k in ("pos", "vel", "mass"))
+    acc = torch.empty_like(pos)
+    out16 = torch.empty(16, dtype=torch.float64, device="cuda")
+    ppgrav.pp_step_kdk(pos, vel, mass, acc, dt, 0, G=G, delta=delta)            # a(t0)
+    series, times = [], []
+
+    def sample(t):
+        ppgrav.pp_invariants(pos, vel, mass, G=G, delta=delta, pot=None, out16=out16)
+        series.append(out16.cpu().numpy().copy())
+        times.append(t)
+
+    sample(0.0)
+    t_wall = time.perf_counter()
+    done = 0
+    while done < steps:
+        n = min(sample_every, steps - done)
+        ppgrav.pp_step_kdk(pos, vel, mass, acc, dt, n, G=G, delta=delta, acc_valid=True)
+        done += n
+        sample(done * dt)
+        if verbose and (done // sample_every) % 10 == 0:
+            s = np.array(series)
+            print("[%s N=2^%d] step %d  dE/E0 %.3e  |dP| %.3e" % (precision, logn, done,
+                  abs(s[-1, 0] - s[0, 0]) / abs(s[0, 0]), np.linalg.norm(s[-1, 3:6] - s[0, 3:6])), flush=True)
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - t_wall
+    s = np.array(series)
+    E, P, L, C = s[:, 0], s[:, 3:6], s[:, 6:9], s[:, 9:12]
+    drift = {
+        "dE_over_E0_max": float(np.max(np.abs(E - E[0])) / abs(E[0])),
+        "dP_abs_max": float(np.max(np.linalg.norm(P - P[0], axis=1))),
+        "dLz_over_Lz0_max": float(np.max(np.abs(L[:, 2] - L[0, 2])) / abs(L[0, 2])),
+        "dCOM_abs_max": float(np.max(np.linalg.norm(C - C[0], axis=1))),
+        "two_K_over_W_first_last": [float(-2 * s[0, 1] / s[0, 2]), float(-2 * s[-1, 1] / s[-1, 2])],
+    }
+    return {"N": N, "precision": precision, "steps": steps, "dt": dt, "t_end": steps * dt,
+            "sample_every": sample_every, "workload": "configs[%d] recipe (%s), seed %d, delta %g" %
+            (config_index, c["name"], c["seed"], delta), "wall_seconds": wall,
+            "pairs_per_second_incl_diagnostics": float(N) * (N - 1) * steps / wall, "drift": drift,
+            "times": times, "E": E.tolist(), "P": P.tolist(), "Lz": L[:, 2].tolist(), "COM": C.tolist()}
+
+
+def main():
+    ap = argparse.ArgumentParser(description=__doc__.split("\n")[0])
+    ap.add_argument("--logn", type=int, nargs="+", default=[17])
+    ap.add_argument("--steps", type=int, default=10000)
+    ap.add_argument("--dt", type=float, default=5e-4)
+    ap.add_argument("--sample-every", type=int, default=100)
+    ap.add_argument("--precision", default="both", choices=["f32", "f64", "both"])
+    ap.add_argument("--out", default=None)
+    a = ap.parse_args()
+    runs = []
+    for logn in a.logn:
+        for prec in (("f32", "f64") if a.precision == "both" else (a.precision,)):
+            r = run(logn, a.steps, a.dt, a.sample_every, prec)
+            print(json.dumps({k: r[k] for k in ("N", "precision", "steps", "dt", "wall_seconds", "drift")}), flush=True)
+            runs.append(r)
+            if a.out:                                   # rewritten after every run: a cut-off job keeps what finished
+                with open(a.out, "w") as f:
+                    json.dump(runs, f)
+    return runs
+
+
+if __name__ == "__main__":
+    main()
