@@ -6,7 +6,8 @@ module.  It imports nothing from the CUDA package and the CUDA package imports n
 Every function takes and returns float64 numpy arrays (row-major [N,3] positions / velocities / accelerations,
 [N] masses) and follows the paper's definitions cited in pp_oracle.cpp:
 forces -> eq. (1)-(2) PAPER.md:41-48; kdk_paper -> eqs. (5)-(7) PAPER.md:67-92; invariants -> eqs. (8)-(10)
-PAPER.md:148-156.
+PAPER.md:148-156; surface_density -> the maps of Fig. 7, PAPER.md:180 (pinned in tests/test_oracle_density.py by a
+hand example, mass conservation, numpy.histogram2d and the analytic exponential profile).
 """
 import ctypes
 import os
@@ -132,3 +133,20 @@ def invariants(pos, vel, mass, G=1.0, delta=0.0, pot=None, nthreads=1):
     d["COM"] = out[9:12].copy()
     d["raw"] = out
     return d
+
+
+def surface_density(pos, mass, x0, y0, cell, nx, ny):
+    """Face-on surface-density map of Fig. 7: sigma[iy, ix] = (sum of m_i over the bodies with
+    x0 + ix*cell <= x_i < x0 + (ix+1)*cell and y0 + iy*cell <= y_i < y0 + (iy+1)*cell) / cell^2, z ignored; bodies
+    outside the nx x ny grid are dropped.  Plain loop over the bodies in index order, float64.  The cell index is
+    floor((x - x0) * (1/cell)) evaluated in float64 -- the one place where floating point decides an integer."""
+    pos = _f64(pos)
+    mass = _f64(mass, (pos.shape[0],))
+    inv = 1.0 / float(cell)
+    sigma = np.zeros((int(ny), int(nx)), dtype=np.float64)
+    for i in range(pos.shape[0]):
+        ix = int(np.floor((pos[i, 0] - x0) * inv))
+        iy = int(np.floor((pos[i, 1] - y0) * inv))
+        if 0 <= ix < nx and 0 <= iy < ny:
+            sigma[iy, ix] += mass[i]
+    return sigma / (float(cell) * float(cell))

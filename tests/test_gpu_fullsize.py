@@ -61,10 +61,17 @@ def _sampled_force_check(gpu, oracle, c, prec, want_pot, tag):
     idx = workloads.sample_indices(c["seed"], c["N"], 4096)
     a_ref, p_ref = oracle.forces(pos, mass, G=c["G"], delta=c["delta"], idx=idx, want_pot=True, nthreads=0)
     dpos, dmass = _dev(prec, pos), _dev(prec, mass)
+    import torch
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
     acc, pot = gpu.pp_forces(dpos, dmass, G=c["G"], delta=c["delta"], want_pot=want_pot)
+    e1.record()
+    torch.cuda.synchronize()
     ea = _rel_rows(acc[idx].cpu().numpy(), a_ref)
+    ms = e0.elapsed_time(e1)           # a single cold call (workspace allocation included): reported, not a bench
     rec = {"N": c["N"], "acc_err_max": float(ea.max()), "acc_err_median": float(np.median(ea)),
-           "acc_err_p999": float(np.quantile(ea, 0.999))}
+           "acc_err_p999": float(np.quantile(ea, 0.999)), "solve_ms": ms, "with_pot": bool(want_pot),
+           "pairs_per_s": float(c["N"]) * (c["N"] - 1) / (ms * 1e-3)}
     assert ea.max() <= TOL[prec], rec
     if want_pot:
         ep = _rel_rows(pot[idx].cpu().numpy(), p_ref)
