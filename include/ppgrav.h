@@ -17,7 +17,8 @@
  *   - _host variants take HOST pointers (pageable or pinned), copy in, run the same kernels, copy out and
  *     synchronise `stream` before returning.
  *   - Layout: pos, vel, acc are row-major [N,3]; mass, pot are [N]; element type float (PP_F32) or double
- *     (PP_F64) according to `precision`; pointers must be aligned to the element size.  No padding is required.
+ *     (PP_F64, PP_MIXED) according to `precision`; pointers must be aligned to the element size.  No padding is
+ *     required.
  *   - delta is the Plummer softening length of PAPER.md:48 (delta >= 0).  delta == 0 is legal: pairs at zero
  *     distance (including padding and j == i) then contribute nothing.
  *   - G multiplies the finished sums once (acc = G * sum), not every pair.
@@ -41,6 +42,11 @@ extern "C" {
 /* precision */
 #define PP_F32 0
 #define PP_F64 1
+/* Extension, not in the paper (motivated by its conclusion): FP64 state and
+ * FP64 time integration, FP32 pair sweep.  Every array is double; each gravity solve rounds the positions and masses
+ * to FP32, runs the PP_F32 sweep (same accuracy as PP_F32: ~1e-7 of |a_i|), and adds and scales its partial sums in
+ * FP64.  What it removes is the rounding of r += dt*v and v += dt/2*a in FP32, at the speed of PP_F32. */
+#define PP_MIXED 2
 
 /* status codes */
 #define PP_OK 0
@@ -119,6 +125,16 @@ int pp_step_kdk(void* pos, void* vel, const void* mass, void* acc, void* pot, in
  *   with compensated accumulation is run on the (promoted) state. */
 int pp_invariants(const void* pos, const void* vel, const void* mass, const void* pot, int64_t N, double G,
                   double delta, int precision, double* out16, void* stream);
+
+/* Face-on surface-density map, the diagnostic of Fig. 7:
+ *   sigma [ny*nx] (device, doubles, row-major, overwritten) = (sum of m_i over the bodies with
+ *   x0 + ix*cell <= x_i < x0 + (ix+1)*cell and y0 + iy*cell <= y_i < y0 + (iy+1)*cell) / cell^2;  z is ignored and
+ *   bodies outside the grid are dropped.  pos [N,3], mass [N] in the state precision; the cell index is
+ *   floor((x - x0) * (1/cell)) evaluated in FP64 on the promoted coordinate.  Sums use floating-point atomics, so
+ *   this diagnostic (unlike the force path) is reproducible only up to summation order (~1e-16 relative).
+ *   PP_EINVAL unless cell > 0, nx, ny >= 1 and nx*ny <= 2^26. */
+int pp_surface_density(const void* pos, const void* mass, int64_t N, double x0, double y0, double cell, int nx,
+                       int ny, int precision, double* sigma, void* stream);
 
 /* Host-buffer variants: same semantics, HOST pointers, synchronous (copies in, computes, copies out). */
 int pp_forces_host(const void* pos, const void* mass, void* acc, void* pot, int64_t N, double G, double delta,

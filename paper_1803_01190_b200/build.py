@@ -13,7 +13,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(ROOT, "include")
 LIB = os.path.join(HERE, "libppgrav.so")
-SOURCES = ("api.cu", "api_host.cu", "plan.cu", "update.cu", "invariants.cu", "force_f32.cu", "force_f64.cu",
+SOURCES = ("api.cu", "api_host.cu", "plan.cu", "update.cu", "invariants.cu", "density.cu", "force_f32.cu", "force_f64.cu",
            "probe.cu")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
               "--ftz=false", "--prec-div=true", "--prec-sqrt=true", "--fmad=true"]

@@ -27,10 +27,11 @@ def run(logn, steps, dt, sample_every, precision, config_index=2, verbose=True):
     c = workloads.config(config_index, N=N)
     G, delta = c["G"], c["delta"]
     dtype = torch.float32 if precision == "f32" else torch.float64
+    mixed = precision == "mixed"                       # FP64 state, FP32 sweep (PP_MIXED)
     pos, vel, mass = (torch.tensor(c[k], dtype=dtype, device="cuda") for k in ("pos", "vel", "mass"))
     acc = torch.empty_like(pos)
     out16 = torch.empty(16, dtype=torch.float64, device="cuda")
-    ppgrav.pp_step_kdk(pos, vel, mass, acc, dt, 0, G=G, delta=delta)            # a(t0)
+    ppgrav.pp_step_kdk(pos, vel, mass, acc, dt, 0, G=G, delta=delta, mixed=mixed)     # a(t0)
     series, times = [], []
 
     def sample(t):
@@ -43,7 +44,7 @@ def run(logn, steps, dt, sample_every, precision, config_index=2, verbose=True):
     done = 0
     while done < steps:
         n = min(sample_every, steps - done)
-        ppgrav.pp_step_kdk(pos, vel, mass, acc, dt, n, G=G, delta=delta, acc_valid=True)
+        ppgrav.pp_step_kdk(pos, vel, mass, acc, dt, n, G=G, delta=delta, acc_valid=True, mixed=mixed)
         done += n
         sample(done * dt)
         if verbose and (done // sample_every) % 10 == 0:
@@ -74,12 +75,13 @@ def main():
     ap.add_argument("--steps", type=int, default=10000)
     ap.add_argument("--dt", type=float, default=5e-4)
     ap.add_argument("--sample-every", type=int, default=100)
-    ap.add_argument("--precision", default="both", choices=["f32", "f64", "both"])
+    ap.add_argument("--precision", default="both", choices=["f32", "f64", "mixed", "both", "all"],
+                    help="both = f32 and f64 (the paper's SP and DP); all adds mixed (FP64 state, FP32 sweep)")
     ap.add_argument("--out", default=None)
     a = ap.parse_args()
     runs = []
     for logn in a.logn:
-        for prec in (("f32", "f64") if a.precision == "both" else (a.precision,)):
+        for prec in {"both": ("f32", "f64"), "all": ("f32", "mixed", "f64")}.get(a.precision, (a.precision,)):
             r = run(logn, a.steps, a.dt, a.sample_every, prec)
             print(json.dumps({k: r[k] for k in ("N", "precision", "steps", "dt", "wall_seconds", "drift")}), flush=True)
             runs.append(r)

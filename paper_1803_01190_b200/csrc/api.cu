@@ -81,8 +81,8 @@ int ensure(Workspace* w, int which, size_t bytes, void** out) {
 bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) & (a - 1)) == 0; }
 
 int check_common(const char* fn, int64_t N, double G, double delta, int precision) {
-    if (precision != PP_F32 && precision != PP_F64) {
-        set_error("%s: precision must be PP_F32 or PP_F64 (got %d)", fn, precision);
+    if (precision != PP_F32 && precision != PP_F64 && precision != PP_MIXED) {
+        set_error("%s: precision must be PP_F32, PP_F64 or PP_MIXED (got %d)", fn, precision);
         return PP_EINVAL;
     }
     if (N < 1 || N > kMaxN) {
@@ -102,7 +102,7 @@ int check_ptr(const char* fn, const char* name, const void* p, int precision, bo
         set_error("%s: %s is NULL", fn, name);
         return PP_EINVAL;
     }
-    if (!aligned(p, precision == PP_F64 ? 8 : 4)) {
+    if (!aligned(p, precision == PP_F32 ? 4 : 8)) {
         set_error("%s: %s is not aligned to its element size", fn, name);
         return PP_EINVAL;
     }
@@ -115,7 +115,9 @@ int check_ptr(const char* fn, const char* name, const void* p, int precision, bo
         if (rc__ != PP_OK) return rc__; \
     } while (0)
 
-size_t elem_bytes(int precision) { return precision == PP_F64 ? 8 : 4; }
+// precision of the pair sweep (packed copy, partial sums): PP_MIXED keeps an FP64 state but sweeps in FP32
+int sweep_precision(int precision) { return precision == PP_F64 ? PP_F64 : PP_F32; }
+size_t sweep_elem_bytes(int precision) { return precision == PP_F64 ? 8 : 4; }
 
 // the pair sweep, optionally bracketed by events (PP_CFG_PROFILE)
 int sweep(const Plan& p, int precision, const void* packed, void* partial, int64_t N, double delta, int mode,
@@ -127,7 +129,7 @@ int sweep(const Plan& p, int precision, const void* packed, void* partial, int64
         PP_CUDA(cudaEventCreate(&e1));
         PP_CUDA(cudaEventRecord(e0, st));
     }
-    const int rc = precision == PP_F32
+    const int rc = sweep_precision(precision) == PP_F32
                        ? launch_force_f32(p, (const float*)packed, (float4*)partial, N, delta, mode, st)
                        : launch_force_f64(p, (const double*)packed, (double4*)partial, N, delta, mode, st);
     if (prof) {
@@ -146,6 +148,9 @@ int solve_packed(const Plan& p, int precision, const void* packed, void* partial
     if (precision == PP_F32)
         return launch_finalize_f32((const float4*)partial, p.split, p.part_stride, p.i_count, G, (float*)acc,
                                    (float*)pot, (float*)vel, kick, st);
+    if (precision == PP_MIXED)
+        return launch_finalize_mixed((const float4*)partial, p.split, p.part_stride, p.i_count, G, (double*)acc,
+                                     (double*)pot, (double*)vel, kick, st);
     return launch_finalize_f64((const double4*)partial, p.split, p.part_stride, p.i_count, G, (double*)acc,
                                (double*)pot, (double*)vel, kick, 0, st);
 }
@@ -153,6 +158,8 @@ int solve_packed(const Plan& p, int precision, const void* packed, void* partial
 int pack_state(int precision, const void* pos, const void* mass, void* packed, int64_t N, int64_t n_pad,
                cudaStream_t st) {
     if (precision == PP_F32) return launch_pack_f32((const float*)pos, (const float*)mass, (float*)packed, N, n_pad, st);
+    if (precision == PP_MIXED)
+        return launch_pack_f64_to_f32((const double*)pos, (const double*)mass, (float*)packed, N, n_pad, st);
     return launch_pack_f64((const double*)pos, (const double*)mass, (double*)packed, N, n_pad, st);
 }
 
@@ -161,14 +168,17 @@ int kick_drift_pack(int precision, void* pos, void* vel, const void* acc, const 
     if (precision == PP_F32)
         return launch_kick_drift_pack_f32((float*)pos, (float*)vel, (const float*)acc, (const float*)mass,
                                           (float*)packed, N, n_pad, kick, dt, st);
+    if (precision == PP_MIXED)
+        return launch_kick_drift_pack_mixed((double*)pos, (double*)vel, (const double*)acc, (const double*)mass,
+                                            (float*)packed, N, n_pad, kick, dt, st);
     return launch_kick_drift_pack_f64((double*)pos, (double*)vel, (const double*)acc, (const double*)mass,
                                       (double*)packed, N, n_pad, kick, dt, st);
 }
 
 int prepare_solve(Workspace* w, int64_t N, int precision, Plan* plan, void** packed, void** partial,
                   int64_t i_begin = 0, int64_t i_count = -1) {
-    *plan = make_plan(N, precision, w->sm_count, g_cfg_split.load(), i_begin, i_count);
-    const size_t body = 4 * elem_bytes(precision);
+    *plan = make_plan(N, sweep_precision(precision), w->sm_count, g_cfg_split.load(), i_begin, i_count);
+    const size_t body = 4 * sweep_elem_bytes(precision);
     PP_TRY(ensure(w, B_PACKED, (size_t)plan->n_pad * body, packed));
     PP_TRY(ensure(w, B_PARTIAL, (size_t)plan->split * (size_t)plan->part_stride * body, partial));
     return PP_OK;
@@ -269,6 +279,7 @@ int pp_plan_query(int64_t N, int precision, int with_pot, int64_t* out8) {
         if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) sm = v;
     }
     cudaGetLastError();
+    precision = sweep_precision(precision);
     const Plan p = make_plan(N, precision, sm, g_cfg_split.load());
     out8[0] = p.i_per_cta;
     out8[1] = p.tile_j;
@@ -393,6 +404,27 @@ int pp_step_kdk(void* pos, void* vel, const void* mass, void* acc, void* pot, in
     }
     PP_TRY(kick_drift_pack(precision, pos, vel, acc, mass, packed, N, plan.n_pad, half, dt, st));
     return solve_packed(plan, precision, packed, partial, N, G, delta, acc, pot, vel, half, st);
+}
+
+int pp_surface_density(const void* pos, const void* mass, int64_t N, double x0, double y0, double cell, int nx,
+                       int ny, int precision, double* sigma, void* stream) {
+    PP_TRY(check_common("pp_surface_density", N, 1.0, 0.0, precision));
+    PP_TRY(check_ptr("pp_surface_density", "pos", pos, precision, true));
+    PP_TRY(check_ptr("pp_surface_density", "mass", mass, precision, true));
+    PP_TRY(check_ptr("pp_surface_density", "sigma", sigma, PP_F64, true));
+    if (!std::isfinite(x0) || !std::isfinite(y0) || !std::isfinite(cell) || !(cell > 0.0) || nx < 1 || ny < 1 ||
+        (int64_t)nx * ny > ((int64_t)1 << 26)) {
+        set_error("pp_surface_density: need finite x0, y0, cell > 0 and 1 <= nx*ny <= 2^26");
+        return PP_EINVAL;
+    }
+    Workspace* w = nullptr;
+    PP_TRY(current_workspace(&w));
+    cudaStream_t st = (cudaStream_t)stream;
+    if (precision == PP_F32)
+        return launch_density_f32((const float*)pos, (const float*)mass, N, x0, y0, cell, nx, ny, sigma, w->sm_count,
+                                  st);
+    return launch_density_f64((const double*)pos, (const double*)mass, N, x0, y0, cell, nx, ny, sigma, w->sm_count,
+                              st);
 }
 
 int pp_invariants(const void* pos, const void* vel, const void* mass, const void* pot, int64_t N, double G,

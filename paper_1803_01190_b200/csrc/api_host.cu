@@ -45,7 +45,7 @@ struct Stage {   // frees its device blocks (stream-ordered) when it goes out of
     } while (0)
 
 bool host_args_ok(const char* fn, int64_t N, int precision) {
-    if ((precision != PP_F32 && precision != PP_F64) || N < 1 || N > ((int64_t)1 << 28)) {
+    if ((precision != PP_F32 && precision != PP_F64 && precision != PP_MIXED) || N < 1 || N > ((int64_t)1 << 28)) {
         set_error("%s: bad precision (%d) or N (%lld)", fn, precision, (long long)N);
         return false;
     }
@@ -61,7 +61,7 @@ int pp_forces_host(const void* pos, const void* mass, void* acc, void* pot, int6
     if (!host_args_ok("pp_forces_host", N, precision)) return PP_EINVAL;
     if (!pos || !mass || !acc) { set_error("pp_forces_host: NULL pointer"); return PP_EINVAL; }
     cudaStream_t st = (cudaStream_t)stream;
-    const size_t e = precision == PP_F64 ? 8 : 4, n = (size_t)N;
+    const size_t e = precision == PP_F32 ? 4 : 8, n = (size_t)N;
     Stage s(st);
     void *dpos, *dmass, *dacc, *dpot = nullptr;
     PP_TRYH(s.upload(pos, 3 * n * e, &dpos));
@@ -80,7 +80,7 @@ int pp_step_kdk_host(void* pos, void* vel, const void* mass, void* acc, void* po
     if (!host_args_ok("pp_step_kdk_host", N, precision)) return PP_EINVAL;
     if (!pos || !vel || !mass || !acc) { set_error("pp_step_kdk_host: NULL pointer"); return PP_EINVAL; }
     cudaStream_t st = (cudaStream_t)stream;
-    const size_t e = precision == PP_F64 ? 8 : 4, n = (size_t)N;
+    const size_t e = precision == PP_F32 ? 4 : 8, n = (size_t)N;
     Stage s(st);
     void *dpos, *dvel, *dmass, *dacc, *dpot = nullptr;
     PP_TRYH(s.upload(pos, 3 * n * e, &dpos));
@@ -104,7 +104,7 @@ int pp_invariants_host(const void* pos, const void* vel, const void* mass, const
     if (!host_args_ok("pp_invariants_host", N, precision)) return PP_EINVAL;
     if (!pos || !vel || !mass || !out16) { set_error("pp_invariants_host: NULL pointer"); return PP_EINVAL; }
     cudaStream_t st = (cudaStream_t)stream;
-    const size_t e = precision == PP_F64 ? 8 : 4, n = (size_t)N;
+    const size_t e = precision == PP_F32 ? 4 : 8, n = (size_t)N;
     Stage s(st);
     void *dpos, *dvel, *dmass, *dpot = nullptr, *dout;
     PP_TRYH(s.upload(pos, 3 * n * e, &dpos));

@@ -97,6 +97,14 @@ int launch_pack_f32(const float* pos, const float* mass, float* packed, int64_t 
 int launch_pack_f64(const double* pos, const double* mass, double* packed, int64_t N, int64_t n_pad, cudaStream_t st);
 int launch_pack_f32_to_f64(const float* pos, const float* mass, double* packed, int64_t N, int64_t n_pad,
                            cudaStream_t st);
+int launch_pack_f64_to_f32(const double* pos, const double* mass, float* packed, int64_t N, int64_t n_pad,
+                           cudaStream_t st);   // PP_MIXED: FP64 state, FP32 sweep
+
+// PP_MIXED variants of finalize and kick_drift_pack: FP32 partial sums / packed copy, FP64 state
+int launch_finalize_mixed(const float4* partial, int split, int64_t n_pad, int64_t N, double G, double* acc,
+                          double* pot, double* vel, double kick, cudaStream_t st);
+int launch_kick_drift_pack_mixed(double* pos, double* vel, const double* acc, const double* mass, float* packed,
+                                 int64_t N, int64_t n_pad, double kick, double dt, cudaStream_t st);
 
 // partial[s * part_stride + (i - i_begin)] = {sum_x, sum_y, sum_z, sum_pot} over the j-tiles of split s, without G and with the
 // sign convention  sum = sum_j m_j (r_j - r_i) w^3,  sum_pot = sum_j m_j w   (w = (r^2+delta^2)^{-1/2}).
@@ -130,6 +138,12 @@ int launch_invariants_f32(const float* pos, const float* vel, const float* mass,
                           const double* pot64, int64_t N, double* scratch, double* out16, cudaStream_t st);
 int launch_invariants_f64(const double* pos, const double* vel, const double* mass, const double* pot_state,
                           const double* pot64, int64_t N, double* scratch, double* out16, cudaStream_t st);
+
+// Fig. 7 surface-density map (density.cu): sigma[iy * nx + ix] = sum of m in the cell / cell^2
+int launch_density_f32(const float* pos, const float* mass, int64_t N, double x0, double y0, double cell, int nx,
+                       int ny, double* sigma, int sm_count, cudaStream_t st);
+int launch_density_f64(const double* pos, const double* mass, int64_t N, double x0, double y0, double cell, int nx,
+                       int ny, double* sigma, int sm_count, cudaStream_t st);
 
 // pipe microbenchmarks (probe.cu)
 int run_probe(int kind, int64_t iters, int sm_count, double* out4);

@@ -54,23 +54,25 @@ template <> struct Vec4<float> { using type = float4; };
 template <> struct Vec4<double> { using type = double4; };
 
 // POT_DD: partial.x/.y are the hi/lo words of a double-double potential sum (MODE_POT of force_f64.cu)
-template <typename T, bool POT_DD>
+// TP: scalar type of the partial sums (the sweep's precision); T: scalar type of the state (acc, pot, vel).  They
+// differ only in PP_MIXED (FP32 sweep, FP64 state), where the S partial sums are added and scaled in FP64.
+template <typename TP, typename T, bool POT_DD>
 __global__ void __launch_bounds__(kThreads)
-finalize_kernel(const typename Vec4<T>::type* __restrict__ partial, int split, int64_t n_pad, int64_t N, T G,
+finalize_kernel(const typename Vec4<TP>::type* __restrict__ partial, int split, int64_t n_pad, int64_t N, T G,
                 T* __restrict__ acc, T* __restrict__ pot, T* __restrict__ vel, T kick) {
     const int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x;
     if (i >= N) return;
     T sx = 0, sy = 0, sz = 0, sw = 0, cx = 0, cy = 0, cz = 0, cw = 0;
     for (int s = 0; s < split; ++s) {   // fixed order s = 0..S-1: run-to-run deterministic
-        const typename Vec4<T>::type v = partial[(size_t)s * n_pad + i];
+        const typename Vec4<TP>::type v = partial[(size_t)s * n_pad + i];
         if (POT_DD) {
-            comp_add(sx, cx, v.x);
-            comp_add(sx, cx, v.y);
+            comp_add(sx, cx, (T)v.x);
+            comp_add(sx, cx, (T)v.y);
         } else {
-            comp_add(sx, cx, v.x);
-            comp_add(sy, cy, v.y);
-            comp_add(sz, cz, v.z);
-            comp_add(sw, cw, v.w);
+            comp_add(sx, cx, (T)v.x);
+            comp_add(sy, cy, (T)v.y);
+            comp_add(sz, cz, (T)v.z);
+            comp_add(sw, cw, (T)v.w);
         }
     }
     if (POT_DD) {
@@ -87,13 +89,14 @@ finalize_kernel(const typename Vec4<T>::type* __restrict__ partial, int split, i
     }
 }
 
-template <typename T>
+// TK: scalar type of the packed copy (the sweep's precision; float for a double state in PP_MIXED)
+template <typename T, typename TK>
 __global__ void __launch_bounds__(kThreads)
 kick_drift_pack_kernel(T* __restrict__ pos, T* __restrict__ vel, const T* __restrict__ acc,
-                       const T* __restrict__ mass, T* __restrict__ packed, int64_t N, int64_t n_pad, T kick, T dt) {
+                       const T* __restrict__ mass, TK* __restrict__ packed, int64_t N, int64_t n_pad, T kick, T dt) {
     const int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x;
     if (i >= n_pad) return;
-    if (i >= N) { store_packed(packed, i, (T)0, (T)0, (T)0, (T)0); return; }
+    if (i >= N) { store_packed(packed, i, (TK)0, (TK)0, (TK)0, (TK)0); return; }
     T r[3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
@@ -102,7 +105,7 @@ kick_drift_pack_kernel(T* __restrict__ pos, T* __restrict__ vel, const T* __rest
         r[c] = fma(dt, v, pos[3 * i + c]);                       // drift, eq. (6)
         pos[3 * i + c] = r[c];
     }
-    store_packed(packed, i, r[0], r[1], r[2], mass[i]);
+    store_packed(packed, i, (TK)r[0], (TK)r[1], (TK)r[2], (TK)mass[i]);
 }
 
 // the sharded step's own-bodies update: opening half-kick + drift (dt != 0) or closing half-kick alone (dt == 0);
@@ -161,8 +164,17 @@ int launch_pack_f32_to_f64(const float* pos, const float* mass, double* packed, 
 
 int launch_finalize_f32(const float4* partial, int split, int64_t n_pad, int64_t N, double G, float* acc, float* pot,
                         float* vel, double kick, cudaStream_t st) {
-    finalize_kernel<float, false><<<grid_for(N), kThreads, 0, st>>>(partial, split, n_pad, N, (float)G, acc, pot,
-                                                                    kick != 0.0 ? vel : nullptr, (float)kick);
+    finalize_kernel<float, float, false><<<grid_for(N), kThreads, 0, st>>>(partial, split, n_pad, N, (float)G, acc,
+                                                                           pot, kick != 0.0 ? vel : nullptr,
+                                                                           (float)kick);
+    count_launch();
+    PP_CUDA(cudaGetLastError());
+    return PP_OK;
+}
+int launch_finalize_mixed(const float4* partial, int split, int64_t n_pad, int64_t N, double G, double* acc,
+                          double* pot, double* vel, double kick, cudaStream_t st) {
+    finalize_kernel<float, double, false><<<grid_for(N), kThreads, 0, st>>>(partial, split, n_pad, N, G, acc, pot,
+                                                                            kick != 0.0 ? vel : nullptr, kick);
     count_launch();
     PP_CUDA(cudaGetLastError());
     return PP_OK;
@@ -170,10 +182,10 @@ int launch_finalize_f32(const float4* partial, int split, int64_t n_pad, int64_t
 int launch_finalize_f64(const double4* partial, int split, int64_t n_pad, int64_t N, double G, double* acc,
                         double* pot, double* vel, double kick, int pot_is_dd, cudaStream_t st) {
     if (pot_is_dd)
-        finalize_kernel<double, true><<<grid_for(N), kThreads, 0, st>>>(partial, split, n_pad, N, G, nullptr, pot,
+        finalize_kernel<double, double, true><<<grid_for(N), kThreads, 0, st>>>(partial, split, n_pad, N, G, nullptr, pot,
                                                                         nullptr, 0.0);
     else
-        finalize_kernel<double, false><<<grid_for(N), kThreads, 0, st>>>(partial, split, n_pad, N, G, acc, pot,
+        finalize_kernel<double, double, false><<<grid_for(N), kThreads, 0, st>>>(partial, split, n_pad, N, G, acc, pot,
                                                                          kick != 0.0 ? vel : nullptr, kick);
     count_launch();
     PP_CUDA(cudaGetLastError());
@@ -182,7 +194,7 @@ int launch_finalize_f64(const double4* partial, int split, int64_t n_pad, int64_
 
 int launch_kick_drift_pack_f32(float* pos, float* vel, const float* acc, const float* mass, float* packed, int64_t N,
                                int64_t n_pad, double kick, double dt, cudaStream_t st) {
-    kick_drift_pack_kernel<float><<<grid_for(n_pad), kThreads, 0, st>>>(pos, vel, acc, mass, packed, N, n_pad,
+    kick_drift_pack_kernel<float, float><<<grid_for(n_pad), kThreads, 0, st>>>(pos, vel, acc, mass, packed, N, n_pad,
                                                                         (float)kick, (float)dt);
     count_launch();
     PP_CUDA(cudaGetLastError());
@@ -190,8 +202,23 @@ int launch_kick_drift_pack_f32(float* pos, float* vel, const float* acc, const f
 }
 int launch_kick_drift_pack_f64(double* pos, double* vel, const double* acc, const double* mass, double* packed,
                                int64_t N, int64_t n_pad, double kick, double dt, cudaStream_t st) {
-    kick_drift_pack_kernel<double><<<grid_for(n_pad), kThreads, 0, st>>>(pos, vel, acc, mass, packed, N, n_pad, kick,
-                                                                         dt);
+    kick_drift_pack_kernel<double, double><<<grid_for(n_pad), kThreads, 0, st>>>(pos, vel, acc, mass, packed, N, n_pad,
+                                                                                 kick, dt);
+    count_launch();
+    PP_CUDA(cudaGetLastError());
+    return PP_OK;
+}
+int launch_kick_drift_pack_mixed(double* pos, double* vel, const double* acc, const double* mass, float* packed,
+                                 int64_t N, int64_t n_pad, double kick, double dt, cudaStream_t st) {
+    kick_drift_pack_kernel<double, float><<<grid_for(n_pad), kThreads, 0, st>>>(pos, vel, acc, mass, packed, N, n_pad,
+                                                                                kick, dt);
+    count_launch();
+    PP_CUDA(cudaGetLastError());
+    return PP_OK;
+}
+int launch_pack_f64_to_f32(const double* pos, const double* mass, float* packed, int64_t N, int64_t n_pad,
+                           cudaStream_t st) {
+    pack_kernel<double, float><<<grid_for(n_pad), kThreads, 0, st>>>(pos, mass, packed, N, n_pad);
     count_launch();
     PP_CUDA(cudaGetLastError());
     return PP_OK;

@@ -15,7 +15,7 @@ import os
 
 import numpy as np
 
-PP_F32, PP_F64 = 0, 1
+PP_F32, PP_F64, PP_MIXED = 0, 1, 2
 PP_ACC_VALID = 1
 PP_CFG_SPLIT_J, PP_CFG_GRAPH, PP_CFG_PROFILE = 1, 2, 3
 INVARIANT_NAMES = ("E", "K", "W", "Px", "Py", "Pz", "Lx", "Ly", "Lz", "Cx", "Cy", "Cz", "M")
@@ -37,6 +37,7 @@ SIGNATURES = {
     "pp_kick_drift": (_int, [_vp, _vp, _vp, _i64, _dbl, _dbl, _int, _vp]),
     "pp_step_kdk": (_int, [_vp, _vp, _vp, _vp, _vp, _i64, _dbl, _i64, _dbl, _dbl, _int, _u, _vp]),
     "pp_invariants": (_int, [_vp, _vp, _vp, _vp, _i64, _dbl, _dbl, _int, _vp, _vp]),
+    "pp_surface_density": (_int, [_vp, _vp, _i64, _dbl, _dbl, _dbl, _int, _int, _int, _vp, _vp]),
     "pp_forces_host": (_int, [_vp, _vp, _vp, _vp, _i64, _dbl, _dbl, _int, _vp]),
     "pp_step_kdk_host": (_int, [_vp, _vp, _vp, _vp, _vp, _i64, _dbl, _i64, _dbl, _dbl, _int, _u, _vp]),
     "pp_invariants_host": (_int, [_vp, _vp, _vp, _vp, _i64, _dbl, _dbl, _int, _vp, _vp]),
@@ -78,8 +79,13 @@ def _torch():
     return torch
 
 
-def _precision_of(t):
+def _precision_of(t, mixed=False):
+    """PP_F32 / PP_F64 from the dtype; mixed=True (float64 arrays only) selects PP_MIXED: FP64 state, FP32 sweep."""
     torch = _torch()
+    if mixed:
+        if t.dtype != torch.float64:
+            raise TypeError("mixed=True needs float64 state arrays, got %s" % t.dtype)
+        return PP_MIXED
     if t.dtype == torch.float32:
         return PP_F32
     if t.dtype == torch.float64:
@@ -137,11 +143,11 @@ def pp_profile_read():
     return float(out[0]), int(out[1])
 
 
-def pp_forces(pos, mass, G=1.0, delta=0.0, want_pot=False, acc=None, pot=None, stream=None):
+def pp_forces(pos, mass, G=1.0, delta=0.0, want_pot=False, acc=None, pot=None, stream=None, mixed=False):
     """Accelerations (and potentials) of all bodies.  pos [N,3], mass [N]: CUDA tensors of one dtype.
     Returns (acc [N,3], pot [N] or None); pass acc/pot to reuse buffers."""
     torch = _torch()
-    prec = _precision_of(pos)
+    prec = _precision_of(pos, mixed)
     N = pos.shape[0]
     p_pos = _dev(pos, (N, 3), pos.dtype, "pos")
     p_mass = _dev(mass, (N,), pos.dtype, "mass")
@@ -157,11 +163,12 @@ def pp_forces(pos, mass, G=1.0, delta=0.0, want_pot=False, acc=None, pot=None, s
     return acc, pot
 
 
-def pp_forces_range(pos, mass, i_begin, i_count, G=1.0, delta=0.0, want_pot=False, acc=None, pot=None, stream=None):
+def pp_forces_range(pos, mass, i_begin, i_count, G=1.0, delta=0.0, want_pot=False, acc=None, pot=None, stream=None,
+                    mixed=False):
     """Accelerations (and potentials) of bodies [i_begin, i_begin + i_count) against all N bodies.
     Returns (acc [i_count,3], pot [i_count] or None)."""
     torch = _torch()
-    prec = _precision_of(pos)
+    prec = _precision_of(pos, mixed)
     N = pos.shape[0]
     n = int(i_count)
     p_pos = _dev(pos, (N, 3), pos.dtype, "pos")
@@ -189,11 +196,12 @@ def pp_kick_drift(pos, vel, acc, kick, dt, stream=None):
                                    _stream(stream)), "pp_kick_drift")
 
 
-def pp_step_kdk(pos, vel, mass, acc, dt, nsteps, G=1.0, delta=0.0, acc_valid=False, pot=None, stream=None):
+def pp_step_kdk(pos, vel, mass, acc, dt, nsteps, G=1.0, delta=0.0, acc_valid=False, pot=None, stream=None,
+                mixed=False):
     """nsteps KDK steps in place on CUDA tensors pos, vel [N,3], mass [N], acc [N,3]; pot [N] (optional) receives
     the potential of the final state (see include/ppgrav.h)."""
     torch = _torch()
-    prec = _precision_of(pos)
+    prec = _precision_of(pos, mixed)
     N = pos.shape[0]
     ptrs = [_dev(pos, (N, 3), pos.dtype, "pos"), _dev(vel, (N, 3), pos.dtype, "vel"),
             _dev(mass, (N,), pos.dtype, "mass"), _dev(acc, (N, 3), pos.dtype, "acc"),
@@ -217,6 +225,21 @@ def pp_invariants(pos, vel, mass, G=1.0, delta=0.0, pot=None, out16=None, stream
                                    _dev(mass, (N,), pos.dtype, "mass"), p_pot, N, float(G), float(delta), prec,
                                    _dev(out16, (16,), torch.float64, "out16"), _stream(stream)), "pp_invariants")
     return out16
+
+
+def pp_surface_density(pos, mass, x0, y0, cell, nx, ny, sigma=None, stream=None):
+    """Surface-density map sigma [ny, nx] (CUDA float64) of the bodies, Fig. 7."""
+    torch = _torch()
+    prec = _precision_of(pos)
+    N = pos.shape[0]
+    if sigma is None:
+        sigma = torch.empty((int(ny), int(nx)), dtype=torch.float64, device=pos.device)
+    with torch.cuda.device(pos.device):
+        _check(lib().pp_surface_density(_dev(pos, (N, 3), pos.dtype, "pos"), _dev(mass, (N,), pos.dtype, "mass"), N,
+                                        float(x0), float(y0), float(cell), int(nx), int(ny), prec,
+                                        _dev(sigma, (ny, nx), torch.float64, "sigma"), _stream(stream)),
+               "pp_surface_density")
+    return sigma
 
 
 def invariants_dict(out16):

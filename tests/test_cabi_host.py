@@ -72,7 +72,8 @@ def test_bad_arguments_and_no_device(ppgrav):
     lib = ppgrav.lib()
     out = (ctypes.c_int64 * 8)()
     assert lib.pp_plan_query(0, 0, 0, out) == -1
-    assert lib.pp_plan_query(10, 2, 0, out) == -1
+    assert lib.pp_plan_query(10, 2, 0, out) == 0          # PP_MIXED plans like PP_F32
+    assert lib.pp_plan_query(10, 3, 0, out) == -1
     assert b"precision" in lib.pp_last_error()
     with pytest.raises(ppgrav.PPGravError):
         ppgrav.pp_configure(99, 0)
