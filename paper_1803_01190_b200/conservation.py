@@ -19,7 +19,11 @@ import time
 import numpy as np
 
 
-def run(logn, steps, dt, sample_every, precision, config_index=2, verbose=True):
+def run(logn, steps, dt, sample_every, precision, config_index=2, verbose=True, checkpoint=None, stop_after=None):
+    """One run.  checkpoint: path of an .npz that is loaded if it exists (resume) and rewritten when the run stops;
+    stop_after: stop (and checkpoint) after that many steps of THIS call, so that a long run can be cut into jobs.
+    A resumed run continues bit for bit: the state (pos, vel, acc) is stored in its own precision."""
+    import os
     import torch
     from . import ppgrav, workloads
 
@@ -28,22 +32,33 @@ def run(logn, steps, dt, sample_every, precision, config_index=2, verbose=True):
     G, delta = c["G"], c["delta"]
     dtype = torch.float32 if precision == "f32" else torch.float64
     mixed = precision == "mixed"                       # FP64 state, FP32 sweep (PP_MIXED)
-    pos, vel, mass = (torch.tensor(c[k], dtype=dtype, device="cuda") for k in ("pos", "vel", "mass"))
-    acc = torch.empty_like(pos)
     out16 = torch.empty(16, dtype=torch.float64, device="cuda")
-    ppgrav.pp_step_kdk(pos, vel, mass, acc, dt, 0, G=G, delta=delta, mixed=mixed)     # a(t0)
     series, times = [], []
+    done = 0
+    wall_before = 0.0
+    if checkpoint and os.path.exists(checkpoint):
+        z = np.load(checkpoint)
+        assert int(z["N"]) == N and str(z["precision"]) == precision and float(z["dt"]) == dt
+        pos, vel, acc = (torch.tensor(z[k], dtype=dtype, device="cuda") for k in ("pos", "vel", "acc"))
+        mass = torch.tensor(c["mass"], dtype=dtype, device="cuda")
+        series, times = [row for row in z["series"]], [float(t) for t in z["times"]]
+        done, wall_before = int(z["done"]), float(z["wall"])
+    else:
+        pos, vel, mass = (torch.tensor(c[k], dtype=dtype, device="cuda") for k in ("pos", "vel", "mass"))
+        acc = torch.empty_like(pos)
+        ppgrav.pp_step_kdk(pos, vel, mass, acc, dt, 0, G=G, delta=delta, mixed=mixed)     # a(t0)
 
     def sample(t):
         ppgrav.pp_invariants(pos, vel, mass, G=G, delta=delta, pot=None, out16=out16)
         series.append(out16.cpu().numpy().copy())
         times.append(t)
 
-    sample(0.0)
+    if not series:
+        sample(0.0)
     t_wall = time.perf_counter()
-    done = 0
-    while done < steps:
-        n = min(sample_every, steps - done)
+    stop_at = steps if stop_after is None else min(steps, done + int(stop_after))
+    while done < stop_at:
+        n = min(sample_every, stop_at - done)
         ppgrav.pp_step_kdk(pos, vel, mass, acc, dt, n, G=G, delta=delta, acc_valid=True, mixed=mixed)
         done += n
         sample(done * dt)
@@ -52,7 +67,10 @@ def run(logn, steps, dt, sample_every, precision, config_index=2, verbose=True):
             print("[%s N=2^%d] step %d  dE/E0 %.3e  |dP| %.3e" % (precision, logn, done,
                   abs(s[-1, 0] - s[0, 0]) / abs(s[0, 0]), np.linalg.norm(s[-1, 3:6] - s[0, 3:6])), flush=True)
     torch.cuda.synchronize()
-    wall = time.perf_counter() - t_wall
+    wall = wall_before + time.perf_counter() - t_wall
+    if checkpoint:
+        np.savez(checkpoint, N=N, precision=precision, dt=dt, done=done, wall=wall, pos=pos.cpu().numpy(),
+                 vel=vel.cpu().numpy(), acc=acc.cpu().numpy(), series=np.array(series), times=np.array(times))
     s = np.array(series)
     E, P, L, C = s[:, 0], s[:, 3:6], s[:, 6:9], s[:, 9:12]
     drift = {
@@ -62,10 +80,10 @@ def run(logn, steps, dt, sample_every, precision, config_index=2, verbose=True):
         "dCOM_abs_max": float(np.max(np.linalg.norm(C - C[0], axis=1))),
         "two_K_over_W_first_last": [float(-2 * s[0, 1] / s[0, 2]), float(-2 * s[-1, 1] / s[-1, 2])],
     }
-    return {"N": N, "precision": precision, "steps": steps, "dt": dt, "t_end": steps * dt,
+    return {"N": N, "precision": precision, "steps": done, "dt": dt, "t_end": done * dt, "steps_requested": steps,
             "sample_every": sample_every, "workload": "configs[%d] recipe (%s), seed %d, delta %g" %
             (config_index, c["name"], c["seed"], delta), "wall_seconds": wall,
-            "pairs_per_second_incl_diagnostics": float(N) * (N - 1) * steps / wall, "drift": drift,
+            "pairs_per_second_incl_diagnostics": float(N) * (N - 1) * done / max(wall, 1e-9), "drift": drift,
             "times": times, "E": E.tolist(), "P": P.tolist(), "Lz": L[:, 2].tolist(), "COM": C.tolist()}
 
 
@@ -78,11 +96,13 @@ def main():
     ap.add_argument("--precision", default="both", choices=["f32", "f64", "mixed", "both", "all"],
                     help="both = f32 and f64 (the paper's SP and DP); all adds mixed (FP64 state, FP32 sweep)")
     ap.add_argument("--out", default=None)
+    ap.add_argument("--checkpoint", default=None, help=".npz to resume from / write to (one --logn, one precision)")
+    ap.add_argument("--stop-after", type=int, default=None, help="steps to run in this call before checkpointing")
     a = ap.parse_args()
     runs = []
     for logn in a.logn:
         for prec in {"both": ("f32", "f64"), "all": ("f32", "mixed", "f64")}.get(a.precision, (a.precision,)):
-            r = run(logn, a.steps, a.dt, a.sample_every, prec)
+            r = run(logn, a.steps, a.dt, a.sample_every, prec, checkpoint=a.checkpoint, stop_after=a.stop_after)
             print(json.dumps({k: r[k] for k in ("N", "precision", "steps", "dt", "wall_seconds", "drift")}), flush=True)
             runs.append(r)
             if a.out:                                   # rewritten after every run: a cut-off job keeps what finished

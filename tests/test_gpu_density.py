@@ -1,6 +1,6 @@
 """GPU parity of pp_surface_density (Fig. 7) against oracle.surface_density on the same seeded bodies:
 identical cell decisions (both sides take floor((x - x0)/cell) in FP64 on what the run actually sees), cell sums equal
-up to summation order."""
+up to summation order (1e-12 of the fullest cell)."""
 import numpy as np
 import pytest
 
@@ -29,7 +29,9 @@ def _run(gpu, oracle, prec, pos, mass, x0, y0, cell, nx, ny):
     ref = oracle.surface_density(seen_p, seen_m, x0, y0, cell, nx, ny)
     assert got.shape == ref.shape == (ny, nx)
     assert np.array_equal(got == 0.0, ref == 0.0), "a body landed in a different cell"
-    assert np.abs(got - ref).max() <= 1e-13 * max(ref.max(), 1e-300)
+    # a cell holds up to n bodies; two summation orders of n positive terms differ by <= n eps (typically sqrt(n) eps),
+    # and the kernel scales each mass by 1/cell^2 before adding where the oracle divides the sum: 30000 eps = 7e-12
+    assert np.abs(got - ref).max() <= 1e-12 * max(ref.max(), 1e-300)
     return got, ref
 
 
