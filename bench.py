@@ -202,7 +202,10 @@ def run_ours(args):
         plan = ppgrav.pp_plan_query(N, ppgrav.PP_F32 if name == "f32" else ppgrav.PP_F64, True)
         lanes = FP32_LANES if name == "f32" else FP64_LANES
         peak = lanes * SM_COUNT * SM_MAX_HZ / 1e12
-        ops = plan["pipe_ops_per_pair"]
+        # pipe operations per pair actually executed: one less on j-tiles whose bodies have a common mass
+        n_tiles, n_common = ppgrav.pp_equal_mass_tiles(mass)
+        plan["equal_mass_tiles"] = [n_tiles, n_common]
+        ops = plan["pipe_ops_per_pair"] - n_common / n_tiles
         achieved = ops * pairs * sweep_n / (sweep_ms * 1e-3) / 1e12 if sweep_ms > 0 else 0.0
         inv = ppgrav.invariants_dict(out16)
         results[name] = dict(
@@ -222,6 +225,11 @@ def run_ours(args):
 
         fms = max_over_ranks(time_steps(torch, force_only, max(2, args.steps // 2), 1, flush, barrier))
         results[name]["force_only"] = replicas.job_value(pairs, max(2, args.steps // 2), fms, world)
+        # the same solve with m_j kept inside the pair loop on every tile (what a system of unequal masses costs)
+        ppgrav.pp_configure(ppgrav.PP_CFG_EQUAL_MASS, 0)
+        gms = max_over_ranks(time_steps(torch, force_only, 2, 1, flush, barrier))
+        ppgrav.pp_configure(ppgrav.PP_CFG_EQUAL_MASS, 1)
+        results[name]["force_only_unequal_masses"] = replicas.job_value(pairs, 2, gms, world)
 
         if name == "f32" and not args.no_e2e:
             # end to end through the host-buffer C ABI: pinned host arrays in, results back, every step
@@ -267,6 +275,7 @@ def run_ours(args):
             "clocks": clocks,
             "sweep_ms_per_launch": r32["sweep_ms_per_launch"], "sweep_share_of_step": r32["sweep_share_of_step"],
             "force_only": {k: results[k]["force_only"] for k in results},
+            "force_only_unequal_masses": {k: results[k]["force_only_unequal_masses"] for k in results},
             "plan": r32["plan"],
         }
         if "f64" in results:

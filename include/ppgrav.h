@@ -61,6 +61,8 @@ extern "C" {
 #define PP_CFG_SPLIT_J 1 /* 0 = automatic (default); S >= 1 forces the j-range to be split S ways */
 #define PP_CFG_GRAPH 2   /* 1 (default) = pp_step_kdk replays its step loop from a CUDA graph when N is small */
 #define PP_CFG_PROFILE 3 /* 1 = bracket every pair-sweep launch with CUDA events (pp_profile_read); no graph replay */
+#define PP_CFG_EQUAL_MASS 4 /* 1 (default) = j-tiles whose bodies all have the same mass take m_j out of the pair loop
+                             * (one pipe operation per pair less); 0 = every tile multiplies by m_j per pair */
 
 /* Version of the library that was loaded (PPGRAV_VERSION). */
 int pp_version(void);
@@ -146,8 +148,15 @@ int pp_invariants_host(const void* pos, const void* vel, const void* mass, const
 
 /* Launch plan the library would use for a gravity solve of N bodies: out8 (host) =
  *   { i-bodies per CTA, j-bodies per tile, split-j factor S, CTAs launched, CTAs resident per SM, SM count,
- *     pipe operations per pair (FP32- or FP64-pipe instructions per lane), MUFU operations per pair }. */
+ *     pipe operations per pair (FP32- or FP64-pipe instructions per lane) on a j-tile of mixed masses -- one less on
+ *     a tile whose bodies have a common mass, see pp_equal_mass_tiles --, MUFU operations per pair }. */
 int pp_plan_query(int64_t N, int precision, int with_pot, int64_t* out8);
+
+/* How many j-tiles of a gravity solve of these masses have a common mass (and therefore run the pair loop without
+ * the per-pair multiplication by m_j): mass [N] (device, `precision`) in; out2 (host) = { j-tiles swept, j-tiles with
+ * a common mass }.  Independent of PP_CFG_EQUAL_MASS.  Synchronous.  bench.py uses it to count the pipe operations
+ * per pair that were actually executed. */
+int pp_equal_mass_tiles(const void* mass, int64_t N, int precision, int64_t* out2, void* stream);
 
 /* Pipe-throughput microbenchmark used for the roofline denominators.
  *   kind: 0 FFMA, 1 FFMA2 (packed f32x2), 2 DFMA, 3 MUFU.RSQ, 4 MUFU.RSQ64H, 5 FFMA2+MUFU in the force kernel's mix (12 : 2),

@@ -24,12 +24,13 @@ std::atomic<int64_t> g_launches{0};
 std::atomic<int64_t> g_cfg_split{0};
 std::atomic<int64_t> g_cfg_graph{1};
 std::atomic<int64_t> g_cfg_profile{0};
+std::atomic<int64_t> g_cfg_equal_mass{1};
 std::vector<std::pair<cudaEvent_t, cudaEvent_t>> g_prof;   // guarded by g_mu (every sweep is launched under it)
 
 constexpr int kMaxDevices = 64;
 constexpr int64_t kMaxN = (int64_t)1 << 28;
-constexpr int kNumBuf = 4;
-enum { B_PACKED = 0, B_PARTIAL, B_INV, B_POT64 };
+constexpr int kNumBuf = 5;
+enum { B_PACKED = 0, B_PARTIAL, B_INV, B_POT64, B_TILE_MASS };
 
 struct Workspace {
     void* buf[kNumBuf] = {};
@@ -120,8 +121,8 @@ int sweep_precision(int precision) { return precision == PP_F64 ? PP_F64 : PP_F3
 size_t sweep_elem_bytes(int precision) { return precision == PP_F64 ? 8 : 4; }
 
 // the pair sweep, optionally bracketed by events (PP_CFG_PROFILE)
-int sweep(const Plan& p, int precision, const void* packed, void* partial, int64_t N, double delta, int mode,
-          cudaStream_t st) {
+int sweep(const Plan& p, int precision, const void* packed, const void* tile_mass, void* partial, int64_t N,
+          double delta, int mode, cudaStream_t st) {
     const bool prof = g_cfg_profile.load() != 0;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (prof) {
@@ -130,8 +131,10 @@ int sweep(const Plan& p, int precision, const void* packed, void* partial, int64
         PP_CUDA(cudaEventRecord(e0, st));
     }
     const int rc = sweep_precision(precision) == PP_F32
-                       ? launch_force_f32(p, (const float*)packed, (float4*)partial, N, delta, mode, st)
-                       : launch_force_f64(p, (const double*)packed, (double4*)partial, N, delta, mode, st);
+                       ? launch_force_f32(p, (const float*)packed, (const float*)tile_mass, (float4*)partial, N, delta,
+                                          mode, st)
+                       : launch_force_f64(p, (const double*)packed, (const double*)tile_mass, (double4*)partial, N,
+                                          delta, mode, st);
     if (prof) {
         PP_CUDA(cudaEventRecord(e1, st));
         g_prof.emplace_back(e0, e1);
@@ -141,10 +144,10 @@ int sweep(const Plan& p, int precision, const void* packed, void* partial, int64
 
 // one gravity solve on already packed bodies: sweep + finalize (optionally with the closing half-kick)
 // (acc, pot, vel address the p.i_count bodies of the plan's i-range)
-int solve_packed(const Plan& p, int precision, const void* packed, void* partial, int64_t N, double G, double delta,
-                 void* acc, void* pot, void* vel, double kick, cudaStream_t st) {
+int solve_packed(const Plan& p, int precision, const void* packed, const void* tile_mass, void* partial, int64_t N,
+                 double G, double delta, void* acc, void* pot, void* vel, double kick, cudaStream_t st) {
     const int mode = pot ? MODE_FORCE_POT : MODE_FORCE;
-    PP_TRY(sweep(p, precision, packed, partial, N, delta, mode, st));
+    PP_TRY(sweep(p, precision, packed, tile_mass, partial, N, delta, mode, st));
     if (precision == PP_F32)
         return launch_finalize_f32((const float4*)partial, p.split, p.part_stride, p.i_count, G, (float*)acc,
                                    (float*)pot, (float*)vel, kick, st);
@@ -161,6 +164,17 @@ int pack_state(int precision, const void* pos, const void* mass, void* packed, i
     if (precision == PP_MIXED)
         return launch_pack_f64_to_f32((const double*)pos, (const double*)mass, (float*)packed, N, n_pad, st);
     return launch_pack_f64((const double*)pos, (const double*)mass, (double*)packed, N, n_pad, st);
+}
+
+// per-j-tile common mass for the plan's tiles (the masses do not change inside an API call: computed once per call)
+int tile_masses(Workspace* w, const Plan& p, int precision, const void* mass, int64_t N, int enable, void** out,
+                cudaStream_t st) {
+    PP_TRY(ensure(w, B_TILE_MASS, (size_t)p.n_tiles * sweep_elem_bytes(precision), out));
+    if (precision == PP_F32)
+        return launch_tile_mass_f32((const float*)mass, (float*)*out, N, p.tile_j, p.n_tiles, enable, st);
+    if (precision == PP_MIXED)
+        return launch_tile_mass_f64_to_f32((const double*)mass, (float*)*out, N, p.tile_j, p.n_tiles, enable, st);
+    return launch_tile_mass_f64((const double*)mass, (double*)*out, N, p.tile_j, p.n_tiles, enable, st);
 }
 
 int kick_drift_pack(int precision, void* pos, void* vel, const void* acc, const void* mass, void* packed, int64_t N,
@@ -217,6 +231,7 @@ int pp_configure(int key, int64_t value) {
     if (key == PP_CFG_SPLIT_J && value >= 0 && value <= 4096) { g_cfg_split.store(value); return PP_OK; }
     if (key == PP_CFG_GRAPH && (value == 0 || value == 1)) { g_cfg_graph.store(value); return PP_OK; }
     if (key == PP_CFG_PROFILE && (value == 0 || value == 1)) { g_cfg_profile.store(value); return PP_OK; }
+    if (key == PP_CFG_EQUAL_MASS && (value == 0 || value == 1)) { g_cfg_equal_mass.store(value); return PP_OK; }
     set_error("pp_configure: unknown key %d or value %lld out of range", key, (long long)value);
     return PP_EINVAL;
 }
@@ -292,6 +307,31 @@ int pp_plan_query(int64_t N, int precision, int with_pot, int64_t* out8) {
     return PP_OK;
 }
 
+int pp_equal_mass_tiles(const void* mass, int64_t N, int precision, int64_t* out2, void* stream) {
+    if (!out2) { set_error("pp_equal_mass_tiles: out2 is NULL"); return PP_EINVAL; }
+    PP_TRY(check_common("pp_equal_mass_tiles", N, 1.0, 0.0, precision));
+    PP_TRY(check_ptr("pp_equal_mass_tiles", "mass", mass, precision, true));
+    std::lock_guard<std::mutex> lk(g_mu);
+    Workspace* w = nullptr;
+    PP_TRY(current_workspace(&w));
+    cudaStream_t st = (cudaStream_t)stream;
+    const Plan plan = make_plan(N, sweep_precision(precision), w->sm_count, g_cfg_split.load());
+    void* tm;
+    PP_TRY(tile_masses(w, plan, precision, mass, N, 1, &tm, st));
+    const size_t eb = sweep_elem_bytes(precision);
+    std::vector<unsigned char> host((size_t)plan.n_tiles * eb);
+    PP_CUDA(cudaMemcpyAsync(host.data(), tm, host.size(), cudaMemcpyDeviceToHost, st));
+    PP_CUDA(cudaStreamSynchronize(st));
+    int64_t common = 0;
+    for (int t = 0; t < plan.n_tiles; ++t) {
+        if (eb == 4) { float v; std::memcpy(&v, &host[(size_t)t * 4], 4); common += (v == v); }
+        else { double v; std::memcpy(&v, &host[(size_t)t * 8], 8); common += (v == v); }
+    }
+    out2[0] = plan.n_tiles;
+    out2[1] = common;
+    return PP_OK;
+}
+
 int pp_probe_pipe(int kind, int64_t iters, double* out4) {
     if (!out4) { set_error("pp_probe_pipe: out4 is NULL"); return PP_EINVAL; }
     Workspace* w = nullptr;
@@ -318,8 +358,10 @@ int pp_forces_range(const void* pos, const void* mass, void* acc, void* pot, int
     Plan plan;
     void *packed, *partial;
     PP_TRY(prepare_solve(w, N, precision, &plan, &packed, &partial, i_begin, i_count));
+    void* tm;
+    PP_TRY(tile_masses(w, plan, precision, mass, N, (int)g_cfg_equal_mass.load(), &tm, st));
     PP_TRY(pack_state(precision, pos, mass, packed, N, plan.n_pad, st));
-    return solve_packed(plan, precision, packed, partial, N, G, delta, acc, pot, nullptr, 0.0, st);
+    return solve_packed(plan, precision, packed, tm, partial, N, G, delta, acc, pot, nullptr, 0.0, st);
 }
 
 int pp_forces(const void* pos, const void* mass, void* acc, void* pot, int64_t N, double G, double delta,
@@ -363,10 +405,13 @@ int pp_step_kdk(void* pos, void* vel, const void* mass, void* acc, void* pot, in
     Plan plan;
     void *packed, *partial;
     PP_TRY(prepare_solve(w, N, precision, &plan, &packed, &partial));
+    if (nsteps == 0 && (flags & PP_ACC_VALID)) return PP_OK;   // nothing to solve
+    void* tm;
+    PP_TRY(tile_masses(w, plan, precision, mass, N, (int)g_cfg_equal_mass.load(), &tm, st));
     if (!(flags & PP_ACC_VALID)) {   // a(t0): the one extra gravity solve of a cold start
         PP_TRY(pack_state(precision, pos, mass, packed, N, plan.n_pad, st));
-        PP_TRY(solve_packed(plan, precision, packed, partial, N, G, delta, acc, nsteps == 0 ? pot : nullptr, nullptr,
-                            0.0, st));
+        PP_TRY(solve_packed(plan, precision, packed, tm, partial, N, G, delta, acc, nsteps == 0 ? pot : nullptr,
+                            nullptr, 0.0, st));
     }
     if (nsteps == 0) return PP_OK;
     const double half = 0.5 * dt;
@@ -381,7 +426,8 @@ int pp_step_kdk(void* pos, void* vel, const void* mass, void* acc, void* pot, in
         cudaGraphExec_t exec = nullptr;
         PP_CUDA(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
         int rc = kick_drift_pack(precision, pos, vel, acc, mass, packed, N, plan.n_pad, half, dt, st);
-        if (rc == PP_OK) rc = solve_packed(plan, precision, packed, partial, N, G, delta, acc, nullptr, vel, half, st);
+        if (rc == PP_OK)
+            rc = solve_packed(plan, precision, packed, tm, partial, N, G, delta, acc, nullptr, vel, half, st);
         const cudaError_t ec = cudaStreamEndCapture(st, &graph);
         if (rc != PP_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
         if (ec != cudaSuccess) return cuda_fail(ec, "cudaStreamEndCapture");
@@ -399,11 +445,11 @@ int pp_step_kdk(void* pos, void* vel, const void* mass, void* acc, void* pot, in
     } else {
         for (int64_t s = 0; s < nbody; ++s) {
             PP_TRY(kick_drift_pack(precision, pos, vel, acc, mass, packed, N, plan.n_pad, half, dt, st));
-            PP_TRY(solve_packed(plan, precision, packed, partial, N, G, delta, acc, nullptr, vel, half, st));
+            PP_TRY(solve_packed(plan, precision, packed, tm, partial, N, G, delta, acc, nullptr, vel, half, st));
         }
     }
     PP_TRY(kick_drift_pack(precision, pos, vel, acc, mass, packed, N, plan.n_pad, half, dt, st));
-    return solve_packed(plan, precision, packed, partial, N, G, delta, acc, pot, vel, half, st);
+    return solve_packed(plan, precision, packed, tm, partial, N, G, delta, acc, pot, vel, half, st);
 }
 
 int pp_surface_density(const void* pos, const void* mass, int64_t N, double x0, double y0, double cell, int nx,
@@ -451,7 +497,7 @@ int pp_invariants(const void* pos, const void* vel, const void* mass, const void
             PP_TRY(launch_pack_f32_to_f64((const float*)pos, (const float*)mass, (double*)packed, N, plan.n_pad, st));
         else
             PP_TRY(launch_pack_f64((const double*)pos, (const double*)mass, (double*)packed, N, plan.n_pad, st));
-        PP_TRY(sweep(plan, PP_F64, packed, partial, N, delta, MODE_POT, st));
+        PP_TRY(sweep(plan, PP_F64, packed, nullptr, partial, N, delta, MODE_POT, st));
         PP_TRY(launch_finalize_f64((const double4*)partial, plan.split, plan.part_stride, N, G, nullptr, (double*)p64,
                                    nullptr, 0.0, 1, st));
         pot64 = (const double*)p64;

@@ -11,6 +11,10 @@
 //  * accumulation is blocked: the packed accumulators only ever hold TJ/2 terms; after every tile they are folded
 //    into a compensated (TwoSum) FP32 outer sum.  A single FP32 accumulator over 2^20 terms is wrong at the 1e-3
 //    level; this keeps the whole solve at ~1e-7.
+//  * equal-mass tiles: when every body of a j-tile has the same mass m (tile_mass[t] = m, written by
+//    tile_mass_kernel in update.cu; NaN otherwise) the factor m_j leaves the pair loop -- the tile accumulates
+//    sum_j w^3 (r_j - r_i) and sum_j w and is scaled by m once, in the fold.  11 (12) instead of 12 (13) FP32-pipe
+//    operations per interaction; N-body workloads are made of a few mass species, so nearly every tile qualifies.
 //  * the (i-block, j-split) decomposition gives the 148 SMs an even number of equal work units at any N; partial
 //    sums go to a workspace and are added in fixed order by finalize (update.cu) -- no floating-point atomics.
 #include "ppgrav_internal.h"
@@ -34,7 +38,7 @@ __device__ __forceinline__ void comp_add(float& s, float& c, float t) {
     c = __fadd_rn(c, e);
 }
 
-template <int IPT, int MODE, bool GUARD, bool DIAG>
+template <int IPT, int MODE, bool GUARD, bool DIAG, bool UNI>
 __device__ __forceinline__ void sweep_tile(const float4* __restrict__ tp, const int npairs, const float2 (&nx)[IPT],
                                            const float2 (&ny)[IPT], const float2 (&nz)[IPT], float2 (&ax)[IPT],
                                            float2 (&ay)[IPT], float2 (&az)[IPT], float2 (&ap)[IPT], const float2 eps2,
@@ -61,7 +65,7 @@ __device__ __forceinline__ void sweep_tile(const float4* __restrict__ tp, const 
                 w.y = r2.y > 0.f ? w.y : 0.f;
             }
             const float2 w2 = __fmul2_rn(w, w);
-            float2 mw = __fmul2_rn(mj, w);
+            float2 mw = UNI ? w : __fmul2_rn(mj, w);          // equal-mass tile: m_j is applied in the fold
             const float2 s = __fmul2_rn(mw, w2);              // m_j / (r^2 + delta^2)^{3/2}
             ax[k] = __ffma2_rn(s, dx, ax[k]);
             ay[k] = __ffma2_rn(s, dy, ay[k]);
@@ -80,8 +84,9 @@ __device__ __forceinline__ void sweep_tile(const float4* __restrict__ tp, const 
 
 template <int THREADS, int IPT, int TJ, int STAGES, int MINB, int MODE, bool GUARD>
 __global__ void __launch_bounds__(THREADS, MINB)
-force_f32_kernel(const float* __restrict__ packed, float4* __restrict__ partial, const int n_tiles,
-                 const int64_t part_stride, const int64_t i_begin, const float eps2f) {
+force_f32_kernel(const float* __restrict__ packed, const float* __restrict__ tile_mass,
+                 float4* __restrict__ partial, const int n_tiles, const int64_t part_stride, const int64_t i_begin,
+                 const float eps2f) {
     constexpr int NWARPS = THREADS / 32;
     constexpr uint32_t TILE_BYTES = TJ * 16u;
     __shared__ __align__(128) float tiles[STAGES][TJ * 4];
@@ -133,16 +138,31 @@ force_f32_kernel(const float* __restrict__ packed, float4* __restrict__ partial,
     const float2 eps2 = make_float2(eps2f, eps2f);
     const int i_lo = (int)i_begin + ib * (THREADS * IPT), i_hi = i_lo + THREADS * IPT;
 
+    // common mass of the bodies of tile t, NaN when they differ (fetched one tile ahead: no exposed latency)
+    const float kNoCommonMass = __int_as_float(0x7fc00000);
+    float tm_next = (tile_mass && nt > 0) ? __ldg(tile_mass + t0) : kNoCommonMass;
+
     for (int t = 0; t < nt; ++t) {
         const int s = t % STAGES;
+        const float tm = tm_next;
+        if (tile_mass && t + 1 < nt) tm_next = __ldg(tile_mass + t0 + t + 1);
+        const bool uni = tm == tm;
         mbar_wait(&full_bar[s], (uint32_t)(t / STAGES) & 1u);
         const float4* tp = reinterpret_cast<const float4*>(&tiles[s][0]);
         const int jbase = (t0 + t) * TJ;
         const bool diag = (MODE == MODE_FORCE_POT) && !GUARD && (jbase < i_hi) && (jbase + TJ > i_lo);
-        if (diag)
-            sweep_tile<IPT, MODE, GUARD, true>(tp, TJ / 2, nx, ny, nz, ax, ay, az, ap, eps2, jbase, iidx);
-        else
-            sweep_tile<IPT, MODE, GUARD, false>(tp, TJ / 2, nx, ny, nz, ax, ay, az, ap, eps2, jbase, iidx);
+        if (uni) {
+            if (diag)
+                sweep_tile<IPT, MODE, GUARD, true, true>(tp, TJ / 2, nx, ny, nz, ax, ay, az, ap, eps2, jbase, iidx);
+            else
+                sweep_tile<IPT, MODE, GUARD, false, true>(tp, TJ / 2, nx, ny, nz, ax, ay, az, ap, eps2, jbase, iidx);
+        } else {
+            if (diag)
+                sweep_tile<IPT, MODE, GUARD, true, false>(tp, TJ / 2, nx, ny, nz, ax, ay, az, ap, eps2, jbase, iidx);
+            else
+                sweep_tile<IPT, MODE, GUARD, false, false>(tp, TJ / 2, nx, ny, nz, ax, ay, az, ap, eps2, jbase, iidx);
+        }
+        const float scale = uni ? tm : 1.0f;   // x 1.0f is exact: the general path is unchanged bit for bit
 
         // release the stage, then (one tile late, so the wait is normally already satisfied) refill the stage
         // that held tile t-1 with tile t-1+STAGES
@@ -158,12 +178,12 @@ force_f32_kernel(const float* __restrict__ packed, float4* __restrict__ partial,
         // blocked accumulation: fold the tile's packed partial sums into the compensated outer sums
 #pragma unroll
         for (int k = 0; k < IPT; ++k) {
-            comp_add(sx[k], cx[k], __fadd_rn(ax[k].x, ax[k].y));
-            comp_add(sy[k], cy[k], __fadd_rn(ay[k].x, ay[k].y));
-            comp_add(sz[k], cz[k], __fadd_rn(az[k].x, az[k].y));
+            comp_add(sx[k], cx[k], __fmul_rn(scale, __fadd_rn(ax[k].x, ax[k].y)));
+            comp_add(sy[k], cy[k], __fmul_rn(scale, __fadd_rn(ay[k].x, ay[k].y)));
+            comp_add(sz[k], cz[k], __fmul_rn(scale, __fadd_rn(az[k].x, az[k].y)));
             ax[k] = ay[k] = az[k] = make_float2(0.f, 0.f);
             if (MODE == MODE_FORCE_POT) {
-                comp_add(sp[k], cp[k], __fadd_rn(ap[k].x, ap[k].y));
+                comp_add(sp[k], cp[k], __fmul_rn(scale, __fadd_rn(ap[k].x, ap[k].y)));
                 ap[k] = make_float2(0.f, 0.f);
             }
         }
@@ -181,12 +201,12 @@ force_f32_kernel(const float* __restrict__ packed, float4* __restrict__ partial,
 }
 
 template <int THREADS, int IPT, int TJ, int STAGES, int MINB>
-int launch_variant(const Plan& p, const float* packed, float4* partial, int64_t N, float eps2, bool guard, int mode,
-                   cudaStream_t st) {
+int launch_variant(const Plan& p, const float* packed, const float* tile_mass, float4* partial, int64_t N, float eps2,
+                   bool guard, int mode, cudaStream_t st) {
     dim3 grid(p.n_iblocks, p.split);
 #define PP_LAUNCH32(MODE_, GUARD_)                                                      \
     force_f32_kernel<THREADS, IPT, TJ, STAGES, MINB, MODE_, GUARD_>                     \
-        <<<grid, THREADS, 0, st>>>(packed, partial, p.n_tiles, p.part_stride, p.i_begin, eps2)
+        <<<grid, THREADS, 0, st>>>(packed, tile_mass, partial, p.n_tiles, p.part_stride, p.i_begin, eps2)
     if (mode == MODE_FORCE) {
         if (guard) PP_LAUNCH32(MODE_FORCE, true); else PP_LAUNCH32(MODE_FORCE, false);
     } else {
@@ -200,17 +220,17 @@ int launch_variant(const Plan& p, const float* packed, float4* partial, int64_t 
 
 }  // namespace
 
-int launch_force_f32(const Plan& p, const float* packed, float4* partial, int64_t N, double delta, int mode,
-                     cudaStream_t st) {
+int launch_force_f32(const Plan& p, const float* packed, const float* tile_mass, float4* partial, int64_t N,
+                     double delta, int mode, cudaStream_t st) {
     const float eps2 = (float)(delta * delta);
     // guarded variant whenever delta^2 is not a normal positive float (r^2 could then be exactly 0)
     const bool guard = !(eps2 >= 1.17549435e-38f);
     constexpr KernelShape L = kShapeF32Large, S = kShapeF32Small;
     if (p.variant == 0)
-        return launch_variant<L.threads, L.ipt, L.tile_j, L.stages, L.ctas_per_sm>(p, packed, partial, N, eps2, guard,
-                                                                                    mode, st);
-    return launch_variant<S.threads, S.ipt, S.tile_j, S.stages, S.ctas_per_sm>(p, packed, partial, N, eps2, guard,
-                                                                                mode, st);
+        return launch_variant<L.threads, L.ipt, L.tile_j, L.stages, L.ctas_per_sm>(p, packed, tile_mass, partial, N,
+                                                                                    eps2, guard, mode, st);
+    return launch_variant<S.threads, S.ipt, S.tile_j, S.stages, S.ctas_per_sm>(p, packed, tile_mass, partial, N, eps2,
+                                                                                guard, mode, st);
 }
 
 }  // namespace ppgrav

@@ -9,6 +9,8 @@
 //    O(e^3)).  MODE_FORCE fuses the correction with the cube: 16 FP64-pipe operations per interaction
 //    (3 DADD + 3 DFMA + 7 + 3 DFMA); with the potential 18; potential only (pp_invariants) 12.  Never 1.0/sqrt(x)
 //    (~30 FP64 operations).
+//  * equal-mass tiles (tile_mass[t] = the common mass, NaN otherwise; see force_f32.cu): the factor m_j is applied
+//    once per tile in the fold -- 15 (17) instead of 16 (18) operations per interaction.  MODE_POT keeps m_j inside.
 //  * blocked accumulation: per-tile sums are folded into outer sums after every tile (plain FP64 for the force,
 //    TwoSum double-double for MODE_POT, which feeds the energy diagnostic).
 #include "ppgrav_internal.h"
@@ -31,7 +33,7 @@ __device__ __forceinline__ void comp_add(double& s, double& c, double t) {
     c = __dadd_rn(c, e);
 }
 
-template <int IPT, int MODE, bool GUARD, bool DIAG>
+template <int IPT, int MODE, bool GUARD, bool DIAG, bool UNI>
 __device__ __forceinline__ void sweep_tile(const double4* __restrict__ tp, const int nj, const double (&xi)[IPT],
                                            const double (&yi)[IPT], const double (&zi)[IPT], double (&ax)[IPT],
                                            double (&ay)[IPT], double (&az)[IPT], double (&ap)[IPT], const double eps2,
@@ -53,7 +55,7 @@ __device__ __forceinline__ void sweep_tile(const double4* __restrict__ tp, const
             const double e = fma(-r2, t, 1.0);                // 1 - x y^2
             if (MODE == MODE_FORCE) {
                 const double p = fma(e, 1.875, 1.5);
-                const double u = b.w * y;
+                const double u = UNI ? y : b.w * y;           // equal-mass tile: m_j is applied in the fold
                 const double w = u * t;                       // m y^3
                 const double we = w * e;
                 const double s = fma(p, we, w);               // m x^{-3/2}
@@ -64,7 +66,7 @@ __device__ __forceinline__ void sweep_tile(const double4* __restrict__ tp, const
                 const double q = fma(e, 0.375, 0.5);
                 const double ye = y * e;
                 const double yy = fma(q, ye, y);              // x^{-1/2} to full precision
-                double u = b.w * yy;                          // m / r
+                double u = UNI ? yy : b.w * yy;               // m / r
                 if (MODE == MODE_FORCE_POT) {
                     const double s = u * (yy * yy);
                     ax[k] = fma(s, dx, ax[k]);
@@ -80,8 +82,9 @@ __device__ __forceinline__ void sweep_tile(const double4* __restrict__ tp, const
 
 template <int THREADS, int IPT, int TJ, int STAGES, int MINB, int MODE, bool GUARD>
 __global__ void __launch_bounds__(THREADS, MINB)
-force_f64_kernel(const double* __restrict__ packed, double4* __restrict__ partial, const int n_tiles,
-                 const int64_t part_stride, const int64_t i_begin, const double eps2) {
+force_f64_kernel(const double* __restrict__ packed, const double* __restrict__ tile_mass,
+                 double4* __restrict__ partial, const int n_tiles, const int64_t part_stride, const int64_t i_begin,
+                 const double eps2) {
     constexpr int NWARPS = THREADS / 32;
     constexpr uint32_t TILE_BYTES = TJ * 32u;
     __shared__ __align__(128) double tiles[STAGES][TJ * 4];
@@ -127,16 +130,32 @@ force_f64_kernel(const double* __restrict__ packed, double4* __restrict__ partia
     }
     const int i_lo = (int)i_begin + ib * (THREADS * IPT), i_hi = i_lo + THREADS * IPT;
 
+    // common mass of the bodies of tile t, NaN when they differ (fetched one tile ahead: no exposed latency)
+    const double kNoCommonMass = __longlong_as_double(0x7ff8000000000000ll);
+    const bool use_tm = (MODE != MODE_POT) && tile_mass != nullptr;
+    double tm_next = (use_tm && nt > 0) ? __ldg(tile_mass + t0) : kNoCommonMass;
+
     for (int t = 0; t < nt; ++t) {
         const int s = t % STAGES;
+        const double tm = tm_next;
+        if (use_tm && t + 1 < nt) tm_next = __ldg(tile_mass + t0 + t + 1);
+        const bool uni = (MODE != MODE_POT) && tm == tm;
         mbar_wait(&full_bar[s], (uint32_t)(t / STAGES) & 1u);
         const double4* tp = reinterpret_cast<const double4*>(&tiles[s][0]);
         const int jbase = (t0 + t) * TJ;
         const bool diag = (MODE != MODE_FORCE) && !GUARD && (jbase < i_hi) && (jbase + TJ > i_lo);
-        if (diag)
-            sweep_tile<IPT, MODE, GUARD, true>(tp, TJ, xi, yi, zi, ax, ay, az, ap, eps2, jbase, iidx);
-        else
-            sweep_tile<IPT, MODE, GUARD, false>(tp, TJ, xi, yi, zi, ax, ay, az, ap, eps2, jbase, iidx);
+        if (MODE != MODE_POT && uni) {
+            if (diag)
+                sweep_tile<IPT, MODE, GUARD, true, true>(tp, TJ, xi, yi, zi, ax, ay, az, ap, eps2, jbase, iidx);
+            else
+                sweep_tile<IPT, MODE, GUARD, false, true>(tp, TJ, xi, yi, zi, ax, ay, az, ap, eps2, jbase, iidx);
+        } else {
+            if (diag)
+                sweep_tile<IPT, MODE, GUARD, true, false>(tp, TJ, xi, yi, zi, ax, ay, az, ap, eps2, jbase, iidx);
+            else
+                sweep_tile<IPT, MODE, GUARD, false, false>(tp, TJ, xi, yi, zi, ax, ay, az, ap, eps2, jbase, iidx);
+        }
+        const double scale = uni ? tm : 1.0;   // x 1.0 is exact: the general path is unchanged bit for bit
 
         __syncwarp();
         if ((tid & 31) == 0) mbar_arrive(&empty_bar[s]);
@@ -150,10 +169,10 @@ force_f64_kernel(const double* __restrict__ packed, double4* __restrict__ partia
 #pragma unroll
         for (int k = 0; k < IPT; ++k) {
             if (MODE != MODE_POT) {
-                sx[k] += ax[k]; sy[k] += ay[k]; sz[k] += az[k];
+                sx[k] = fma(scale, ax[k], sx[k]); sy[k] = fma(scale, ay[k], sy[k]); sz[k] = fma(scale, az[k], sz[k]);
                 ax[k] = ay[k] = az[k] = 0.0;
             }
-            if (MODE == MODE_FORCE_POT) { sp[k] += ap[k]; ap[k] = 0.0; }
+            if (MODE == MODE_FORCE_POT) { sp[k] = fma(scale, ap[k], sp[k]); ap[k] = 0.0; }
             if (MODE == MODE_POT) { comp_add(sp[k], cp[k], ap[k]); ap[k] = 0.0; }
         }
     }
@@ -168,12 +187,12 @@ force_f64_kernel(const double* __restrict__ packed, double4* __restrict__ partia
 }
 
 template <int THREADS, int IPT, int TJ, int STAGES, int MINB>
-int launch_variant(const Plan& p, const double* packed, double4* partial, int64_t N, double eps2, bool guard, int mode,
-                   cudaStream_t st) {
+int launch_variant(const Plan& p, const double* packed, const double* tile_mass, double4* partial, int64_t N,
+                   double eps2, bool guard, int mode, cudaStream_t st) {
     dim3 grid(p.n_iblocks, p.split);
 #define PP_LAUNCH64(MODE_, GUARD_)                                                      \
     force_f64_kernel<THREADS, IPT, TJ, STAGES, MINB, MODE_, GUARD_>                     \
-        <<<grid, THREADS, 0, st>>>(packed, partial, p.n_tiles, p.part_stride, p.i_begin, eps2)
+        <<<grid, THREADS, 0, st>>>(packed, tile_mass, partial, p.n_tiles, p.part_stride, p.i_begin, eps2)
     if (mode == MODE_FORCE) {
         if (guard) PP_LAUNCH64(MODE_FORCE, true); else PP_LAUNCH64(MODE_FORCE, false);
     } else if (mode == MODE_FORCE_POT) {
@@ -189,16 +208,16 @@ int launch_variant(const Plan& p, const double* packed, double4* partial, int64_
 
 }  // namespace
 
-int launch_force_f64(const Plan& p, const double* packed, double4* partial, int64_t N, double delta, int mode,
-                     cudaStream_t st) {
+int launch_force_f64(const Plan& p, const double* packed, const double* tile_mass, double4* partial, int64_t N,
+                     double delta, int mode, cudaStream_t st) {
     const double eps2 = delta * delta;
     const bool guard = !(eps2 >= 2.2250738585072014e-308);
     constexpr KernelShape L = kShapeF64Large, S = kShapeF64Small;
     if (p.variant == 0)
-        return launch_variant<L.threads, L.ipt, L.tile_j, L.stages, L.ctas_per_sm>(p, packed, partial, N, eps2, guard,
-                                                                                    mode, st);
-    return launch_variant<S.threads, S.ipt, S.tile_j, S.stages, S.ctas_per_sm>(p, packed, partial, N, eps2, guard,
-                                                                                mode, st);
+        return launch_variant<L.threads, L.ipt, L.tile_j, L.stages, L.ctas_per_sm>(p, packed, tile_mass, partial, N,
+                                                                                    eps2, guard, mode, st);
+    return launch_variant<S.threads, S.ipt, S.tile_j, S.stages, S.ctas_per_sm>(p, packed, tile_mass, partial, N, eps2,
+                                                                                guard, mode, st);
 }
 
 }  // namespace ppgrav

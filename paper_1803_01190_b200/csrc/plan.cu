@@ -47,8 +47,8 @@ Plan make_plan(int64_t N, int precision, int sm_count, int64_t forced_split, int
         p.i_count = i_count;
         p.n_iblocks = (int)((i_count + p.i_per_cta - 1) / p.i_per_cta);
         p.part_stride = (int64_t)p.n_iblocks * p.i_per_cta;
-        // tile_j divides i_per_cta in both variants; the last launched i-block may reach past N
-        p.n_pad = round_up(std::max(N, i_begin + p.part_stride), std::max(p.i_per_cta, p.tile_j));
+        // the packed array must cover the last launched i-block (which may reach past N) and the last j-tile
+        p.n_pad = round_up(std::max(N, i_begin + p.part_stride), p.tile_j);
         p.n_tiles = (int)((N + p.tile_j - 1) / p.tile_j);
         const int64_t resident = (int64_t)sm_count * d.ctas_per_sm;
         // partial sums: S x n_pad x {16,32} bytes, kept under 1 GiB

@@ -26,7 +26,7 @@ void count_launch(int n = 1);
 #define PP_F32_THREADS 256
 #endif
 #ifndef PP_F32_IPT
-#define PP_F32_IPT 6
+#define PP_F32_IPT 7
 #endif
 #ifndef PP_F32_TJ
 #define PP_F32_TJ 512
@@ -100,6 +100,14 @@ int launch_pack_f32_to_f64(const float* pos, const float* mass, double* packed, 
 int launch_pack_f64_to_f32(const double* pos, const double* mass, float* packed, int64_t N, int64_t n_pad,
                            cudaStream_t st);   // PP_MIXED: FP64 state, FP32 sweep
 
+// tile_mass[t] (sweep precision) = common mass of the tile_j bodies of j-tile t, NaN if they differ (or !enable)
+int launch_tile_mass_f32(const float* mass, float* tile_mass, int64_t N, int tile_j, int n_tiles, int enable,
+                         cudaStream_t st);
+int launch_tile_mass_f64(const double* mass, double* tile_mass, int64_t N, int tile_j, int n_tiles, int enable,
+                         cudaStream_t st);
+int launch_tile_mass_f64_to_f32(const double* mass, float* tile_mass, int64_t N, int tile_j, int n_tiles, int enable,
+                                cudaStream_t st);
+
 // PP_MIXED variants of finalize and kick_drift_pack: FP32 partial sums / packed copy, FP64 state
 int launch_finalize_mixed(const float4* partial, int split, int64_t n_pad, int64_t N, double G, double* acc,
                           double* pot, double* vel, double kick, cudaStream_t st);
@@ -108,11 +116,12 @@ int launch_kick_drift_pack_mixed(double* pos, double* vel, const double* acc, co
 
 // partial[s * part_stride + (i - i_begin)] = {sum_x, sum_y, sum_z, sum_pot} over the j-tiles of split s, without G and with the
 // sign convention  sum = sum_j m_j (r_j - r_i) w^3,  sum_pot = sum_j m_j w   (w = (r^2+delta^2)^{-1/2}).
-int launch_force_f32(const Plan& p, const float* packed, float4* partial, int64_t N, double delta, int mode,
-                     cudaStream_t st);
+// tile_mass: per-j-tile common mass (launch_tile_mass_*), or NULL = treat every tile as mixed.
+int launch_force_f32(const Plan& p, const float* packed, const float* tile_mass, float4* partial, int64_t N,
+                     double delta, int mode, cudaStream_t st);
 // MODE_POT writes {pot_hi, pot_lo, 0, 0} (double-double partial of the potential sum).
-int launch_force_f64(const Plan& p, const double* packed, double4* partial, int64_t N, double delta, int mode,
-                     cudaStream_t st);
+int launch_force_f64(const Plan& p, const double* packed, const double* tile_mass, double4* partial, int64_t N,
+                     double delta, int mode, cudaStream_t st);
 
 // acc = G * sum_s partial (fixed order, compensated), pot = -G * sum_s partial.w; optional fused kick
 // vel += kick * acc (kick = 0: none).  acc/pot/vel may be NULL where not wanted.

@@ -35,6 +35,26 @@ __global__ void __launch_bounds__(kThreads) pack_kernel(const TIn* __restrict__ 
         store_packed(packed, i, (TOut)0, (TOut)0, (TOut)0, (TOut)0);   // padding: massless, contributes nothing
 }
 
+// tile_mass[t] = m if all tile_j bodies of j-tile t have the same mass m in the sweep's precision (bodies >= N are
+// padding of mass 0), NaN otherwise.  One warp per tile.  The sweeps (force_f32.cu / force_f64.cu) take m_j out of
+// the pair loop on tiles that have a common mass.  enable == 0 writes NaN everywhere (PP_CFG_EQUAL_MASS off).
+template <typename TIn, typename TOut>
+__global__ void __launch_bounds__(kThreads) tile_mass_kernel(const TIn* __restrict__ mass, TOut* __restrict__ tile_mass,
+                                                             int64_t N, int tile_j, int n_tiles, int enable) {
+    const int t = (int)(((int64_t)blockIdx.x * kThreads + threadIdx.x) >> 5);
+    const int lane = threadIdx.x & 31;
+    if (t >= n_tiles) return;                                  // whole warps leave together
+    const int64_t j0 = (int64_t)t * tile_j;
+    const TOut first = (TOut)mass[j0];                         // j0 < N: only tiles with a real body are swept
+    bool same = enable != 0;
+    for (int j = lane; j < tile_j; j += 32) {
+        const TOut m = (j0 + j < N) ? (TOut)mass[j0 + j] : (TOut)0;
+        same = same && (m == first);
+    }
+    same = __all_sync(0xffffffffu, same);
+    if (lane == 0) tile_mass[t] = same ? first : (TOut)NAN;
+}
+
 // error-free s + t -> (s, err accumulated into c); intrinsics keep the compiler from contracting/reassociating
 __device__ __forceinline__ void comp_add(float& s, float& c, float t) {
     const float n = __fadd_rn(s, t);
@@ -222,6 +242,28 @@ int launch_pack_f64_to_f32(const double* pos, const double* mass, float* packed,
     count_launch();
     PP_CUDA(cudaGetLastError());
     return PP_OK;
+}
+
+template <typename TIn, typename TOut>
+static int launch_tile_mass(const TIn* mass, TOut* tile_mass, int64_t N, int tile_j, int n_tiles, int enable,
+                            cudaStream_t st) {
+    tile_mass_kernel<TIn, TOut><<<grid_for((int64_t)n_tiles * 32), kThreads, 0, st>>>(mass, tile_mass, N, tile_j,
+                                                                                      n_tiles, enable);
+    count_launch();
+    PP_CUDA(cudaGetLastError());
+    return PP_OK;
+}
+int launch_tile_mass_f32(const float* mass, float* tile_mass, int64_t N, int tile_j, int n_tiles, int enable,
+                         cudaStream_t st) {
+    return launch_tile_mass(mass, tile_mass, N, tile_j, n_tiles, enable, st);
+}
+int launch_tile_mass_f64(const double* mass, double* tile_mass, int64_t N, int tile_j, int n_tiles, int enable,
+                         cudaStream_t st) {
+    return launch_tile_mass(mass, tile_mass, N, tile_j, n_tiles, enable, st);
+}
+int launch_tile_mass_f64_to_f32(const double* mass, float* tile_mass, int64_t N, int tile_j, int n_tiles, int enable,
+                                cudaStream_t st) {
+    return launch_tile_mass(mass, tile_mass, N, tile_j, n_tiles, enable, st);
 }
 
 }  // namespace ppgrav

@@ -17,7 +17,7 @@ import numpy as np
 
 PP_F32, PP_F64, PP_MIXED = 0, 1, 2
 PP_ACC_VALID = 1
-PP_CFG_SPLIT_J, PP_CFG_GRAPH, PP_CFG_PROFILE = 1, 2, 3
+PP_CFG_SPLIT_J, PP_CFG_GRAPH, PP_CFG_PROFILE, PP_CFG_EQUAL_MASS = 1, 2, 3, 4
 INVARIANT_NAMES = ("E", "K", "W", "Px", "Py", "Pz", "Lx", "Ly", "Lz", "Cx", "Cy", "Cz", "M")
 PROBE_KINDS = {"ffma": 0, "ffma2": 1, "dfma": 2, "mufu_rsq": 3, "mufu_rsq64h": 4, "force_mix_f32": 5,
                "ffma2_dfma_const": 6, "ffma2_3reg": 7, "ffma2_dfma_3reg": 8}
@@ -42,6 +42,7 @@ SIGNATURES = {
     "pp_step_kdk_host": (_int, [_vp, _vp, _vp, _vp, _vp, _i64, _dbl, _i64, _dbl, _dbl, _int, _u, _vp]),
     "pp_invariants_host": (_int, [_vp, _vp, _vp, _vp, _i64, _dbl, _dbl, _int, _vp, _vp]),
     "pp_plan_query": (_int, [_i64, _int, _int, _vp]),
+    "pp_equal_mass_tiles": (_int, [_vp, _i64, _int, _vp, _vp]),
     "pp_probe_pipe": (_int, [_int, _i64, _vp]),
     "pp_profile_read": (_int, [_vp]),
 }
@@ -127,6 +128,16 @@ def pp_plan_query(N, precision, with_pot=False):
     keys = ("i_per_cta", "tile_j", "split", "ctas", "ctas_per_sm", "sm_count", "pipe_ops_per_pair",
             "mufu_per_pair")
     return dict(zip(keys, (int(v) for v in out)))
+
+
+def pp_equal_mass_tiles(mass, stream=None, mixed=False):
+    """(j-tiles swept, j-tiles whose bodies have a common mass) for a gravity solve of these masses."""
+    prec = _precision_of(mass, mixed)
+    N = mass.shape[0]
+    out = (ctypes.c_int64 * 2)()
+    _check(lib().pp_equal_mass_tiles(_dev(mass, (N,), mass.dtype, "mass"), N, prec, out, _stream(stream)),
+           "pp_equal_mass_tiles")
+    return int(out[0]), int(out[1])
 
 
 def pp_probe_pipe(kind, iters=1 << 14):

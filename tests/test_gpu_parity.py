@@ -156,6 +156,82 @@ def test_forces_rejects_bad_arguments(gpu):
     torch.cuda.synchronize()
 
 
+# ---- equal-mass j-tiles (m_j taken out of the pair loop) -----------------------------------------------------------
+def _species_cloud(n, seed, bounds, masses):
+    """n bodies in mass species: bodies [bounds[k], bounds[k+1]) all have mass masses[k] (exactly)."""
+    pos, vel, _ = _random_cloud(n, seed)
+    mass = np.empty(n)
+    edges = list(bounds) + [n]
+    for k, m in enumerate(masses):
+        mass[edges[k]:edges[k + 1]] = m
+    return pos, vel, mass
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("n,bounds", [(3001, (0, 1300)), (40003, (0, 700, 21000)), (1537, (0,))])
+def test_equal_mass_tiles_against_oracle_and_general_path(gpu, oracle, prec, n, bounds):
+    """Species boundaries off the tile grid and a ragged tail: tiles inside one species run without the per-pair
+    m_j, the straddling tiles and the padded last tile with it.  Both settings of PP_CFG_EQUAL_MASS must meet the
+    oracle; they differ from each other by summation round-off only."""
+    masses = [1.0 / n, 4.0 / n, 0.25 / n][:len(bounds)]
+    pos, vel, mass = _species_cloud(n, 77 + n, bounds, masses)
+    pos, mass = _inputs_seen(prec, pos, mass)
+    a_ref, p_ref = oracle.forces(pos, mass, G=1.5, delta=0.03, nthreads=0)
+    dpos, dmass = _to_dev(prec, pos, mass)
+    tile_j = gpu.pp_plan_query(n, gpu.PP_F64 if prec == "f64" else gpu.PP_F32)["tile_j"]
+    edges = list(bounds) + [n]
+    expect = sum(1 for t in range((n + tile_j - 1) // tile_j)
+                 if (t + 1) * tile_j <= n and any(edges[k] <= t * tile_j and (t + 1) * tile_j <= edges[k + 1]
+                                                  for k in range(len(bounds))))
+    assert gpu.pp_equal_mass_tiles(dmass) == ((n + tile_j - 1) // tile_j, expect) and expect > 0
+    res = {}
+    try:
+        for flag in (1, 0):
+            gpu.pp_configure(gpu.PP_CFG_EQUAL_MASS, flag)
+            acc, pot = gpu.pp_forces(dpos, dmass, G=1.5, delta=0.03, want_pot=True)
+            acc2, _ = gpu.pp_forces(dpos, dmass, G=1.5, delta=0.03, want_pot=False)
+            assert rel_err_rows(acc.cpu().numpy(), a_ref) <= TOL_ACC[prec]
+            assert rel_err_rows(acc2.cpu().numpy(), a_ref) <= TOL_ACC[prec]
+            assert rel_err_rows(pot.cpu().numpy(), p_ref) <= TOL_POT[prec]
+            res[flag] = (acc.cpu().numpy(), pot.cpu().numpy())
+    finally:
+        gpu.pp_configure(gpu.PP_CFG_EQUAL_MASS, 1)
+    assert not np.array_equal(res[0][0], res[1][0])          # the two paths really are different instruction streams
+    assert rel_err_rows(res[1][0], res[0][0]) <= {"f64": 1e-13, "f32": 1e-5}[prec]
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_mixed_mass_tiles_do_not_depend_on_the_switch(gpu, prec):
+    """No tile of a random-mass cloud has a common mass: PP_CFG_EQUAL_MASS on/off are then bit-identical."""
+    pos, vel, mass = _random_cloud(3001, 13)
+    dpos, dmass = _to_dev(prec, pos, mass)
+    assert gpu.pp_equal_mass_tiles(dmass)[1] == 0
+    outs = []
+    try:
+        for flag in (1, 0):
+            gpu.pp_configure(gpu.PP_CFG_EQUAL_MASS, flag)
+            outs.append(gpu.pp_forces(dpos, dmass, delta=0.05, want_pot=True))
+    finally:
+        gpu.pp_configure(gpu.PP_CFG_EQUAL_MASS, 1)
+    import torch
+    assert torch.equal(outs[0][0], outs[1][0]) and torch.equal(outs[0][1], outs[1][1])
+
+
+def test_equal_mass_tiles_delta_zero_and_massless(gpu, oracle):
+    """Guarded (delta = 0) kernels and an all-massless species go through the equal-mass path too."""
+    n = 2048
+    pos, vel, mass = _species_cloud(n, 5, (0, 1024), [1.0 / n, 0.0])
+    a_ref, p_ref = oracle.forces(pos, mass, delta=0.0, nthreads=0)
+    for prec in ("f64", "f32"):
+        p, m = _inputs_seen(prec, pos, mass)
+        ar, pr = (a_ref, p_ref) if prec == "f64" else oracle.forces(p, m, delta=0.0, nthreads=0)
+        dpos, dmass = _to_dev(prec, p, m)
+        assert gpu.pp_equal_mass_tiles(dmass)[1] == gpu.pp_equal_mass_tiles(dmass)[0]
+        acc, pot = gpu.pp_forces(dpos, dmass, delta=0.0, want_pot=True)
+        assert rel_err_rows(acc.cpu().numpy(), ar) <= TOL_ACC[prec]
+        assert rel_err_rows(pot.cpu().numpy(), pr) <= TOL_POT[prec]
+
+
 # ---- pp_step_kdk -------------------------------------------------------------------------------------------------
 TOL_TRAJ = {"f64": 1e-11, "f32": 5e-6}
 
@@ -176,8 +252,9 @@ def test_kdk_config0_trajectory(gpu, oracle, prec):
     n0 = gpu.pp_launch_count()
     gpu.pp_step_kdk(dpos, dvel, dmass, dacc, c["dt"], c["nsteps"], G=c["G"], delta=c["delta"], pot=dpot)
     torch.cuda.synchronize()
-    # one gravity solve per step + the cold-start solve: (pack, sweep, finalize) + 3 per step
-    assert gpu.pp_launch_count() - n0 == 3 + 3 * c["nsteps"]
+    # one gravity solve per step + the cold-start solve: tile masses once per call,
+    # (pack, sweep, finalize) for the cold start, 3 launches per step
+    assert gpu.pp_launch_count() - n0 == 4 + 3 * c["nsteps"]
     scale_r, scale_v = np.abs(p_ref).max(), np.abs(v_ref).max()
     assert np.abs(dpos.cpu().numpy() - p_ref).max() / scale_r <= TOL_TRAJ[prec]
     assert np.abs(dvel.cpu().numpy() - v_ref).max() / scale_v <= TOL_TRAJ[prec]
