@@ -37,8 +37,8 @@ UNIT = "pair-interactions/s"
 # nominal pipe peaks: lanes per SM x SMs x max SM clock
 FP32_LANES, FP64_LANES, SM_COUNT, SM_MAX_HZ = 128, 64, 148, 1.965e9
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE sweep launch (with potential) at N = 2^20, from the
-# `ncu --set full` captures summarised in profiles/r1_force_f32_ncu.md / profiles/r1_force_f64_ncu.md
-NCU_TRAFFIC_BYTES = {("f32", 1 << 20): 17.068288e6 + 3.349760e6, ("f64", 1 << 20): 43.715584e6 + 57.617664e6}
+# `ncu --set full` captures summarised in profiles/r1d_force_f32_ncu.md / profiles/r1d_force_f64_ncu.md
+NCU_TRAFFIC_BYTES = {("f32", 1 << 20): 17.038848e6 + 0.0, ("f64", 1 << 20): 68.253184e6 + 106.742784e6}
 L2_FLUSH_BYTES = 256 << 20
 
 
