@@ -277,6 +277,8 @@ def run_ours(args):
             "force_only": {k: results[k]["force_only"] for k in results},
             "force_only_unequal_masses": {k: results[k]["force_only_unequal_masses"] for k in results},
             "plan": r32["plan"],
+            # the literature's convention: 20 flop per pair interaction (rsqrt counted as 4), force-only solve
+            "tflops_20_flop_per_pair": {k: 20.0 * results[k]["force_only"] / 1e12 for k in results},
         }
         if "f64" in results:
             r64 = results["f64"]
