@@ -24,6 +24,11 @@ const VariantDesc kVariants[2][2] = {
 
 int64_t round_up(int64_t a, int64_t b) { return (a + b - 1) / b * b; }
 
+// weight of one split-j partial sum of one body (written by the sweep, read by the finalize pass), in pair
+// interactions of one SM.  The bandwidth cost alone is ~0.1; the weight is larger so that a bigger S is only taken when
+// it fills the last wave noticeably better.  Calibrated on the B200 (N = 2^11 .. 2^22 sweep).
+constexpr double kFinalizeCost = 16.0;
+
 }  // namespace
 
 Plan make_plan(int64_t N, int precision, int sm_count, int64_t forced_split, int64_t i_begin, int64_t i_count) {
@@ -62,7 +67,7 @@ Plan make_plan(int64_t N, int precision, int sm_count, int64_t forced_split, int
             const int64_t waves = (units + resident - 1) / resident;
             const int64_t tps = (p.n_tiles + S - 1) / S;
             // 2 tile-times of fixed cost per unit (pipeline fill, epilogue), plus the finalize pass over S partials
-            const double cost = (double)waves * ((double)tps + 2.0) * tile_cost + 64.0 * (double)S * (double)p.part_stride;
+            const double cost = (double)waves * ((double)tps + 2.0) * tile_cost + kFinalizeCost * (double)S * (double)p.part_stride;
             if (best_cost < 0.0 || cost < best_cost * (1.0 - 1e-9)) {
                 best_cost = cost;
                 best = p;
