@@ -50,6 +50,11 @@ def test_plan_is_sane(ppgrav, prec):
         n_pad = -(-n // p["i_per_cta"]) * p["i_per_cta"]
         assert p["split"] * n_pad * elem <= (1 << 30) or p["split"] == 1
         assert p["pipe_ops_per_pair"] == (16 if prec else 12)
+    # calibrated choices: the throughput shape from N = 2^16 up, the small one below 2^14
+    for n in (2 ** 16, 2 ** 17, 2 ** 20, 2 ** 23):
+        assert ppgrav.pp_plan_query(n, prec)["i_per_cta"] >= 1536
+    for n in (100, 2048, 2 ** 13):
+        assert ppgrav.pp_plan_query(n, prec)["i_per_cta"] == 128
     big = ppgrav.pp_plan_query(2 ** 20, prec)
     resident = big["sm_count"] * big["ctas_per_sm"]
     waves = big["ctas"] / resident
