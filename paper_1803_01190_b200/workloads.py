@@ -24,7 +24,8 @@ import math
 import numpy as np
 
 _STREAMS = {"disk_R": 1, "disk_phi": 2, "disk_z": 3, "disk_vel": 4, "plummer_r": 5, "plummer_dir": 6,
-            "plummer_q": 7, "plummer_vdir": 8, "sample": 9}
+            "plummer_q": 7, "plummer_vdir": 8, "sample": 9, "jeans_R": 10, "jeans_phi": 11, "jeans_z": 12,
+            "jeans_vel": 13}
 
 DISK_TRUNC = 4.0          # truncation radius in units of h
 DISK_Z0 = 0.1
@@ -158,6 +159,14 @@ def config(k, N=None):
     c["G"] = 1.0
     c["pos"], c["vel"], c["mass"] = make(c["kind"], c["N"], c["seed"], c.get("sigma_f", 0.1), c["G"])
     return c
+
+
+def jeans_disk_draws(n, seed):
+    """The random numbers of the equilibrium-disk generator of eqs. (3)-(4): uniforms in (0, 1) for
+    radius, azimuth and height, standard normals for the three velocity components.  Both the CUDA-path generator
+    (disk_ic.py) and the oracle's (oracle/disk_ic.py) take these as INPUTS, so neither draws anything itself."""
+    return {"u_R": _open01(_rng(seed, "jeans_R"), n), "u_phi": _open01(_rng(seed, "jeans_phi"), n),
+            "u_z": _open01(_rng(seed, "jeans_z"), n), "g": _rng(seed, "jeans_vel").standard_normal((n, 3))}
 
 
 def sample_indices(seed, N, n=4096):

@@ -1,0 +1,124 @@
+"""Pins of the oracle's equilibrium-disk generator (oracle/disk_ic.py; eqs. (3)-(4)) against what the
+mathematics fixes: the isothermal-sheet closed form of eq. (4), the equation's own residual by finite differences, the
+analytic cumulative mass of the exponential disk, the radial Jeans balance measured from the generated particles, the
+cold-disk limit v_phi^2 = r g_r, and the virial ratio of the result.  CPU only."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import disk_ic, oracle
+from paper_1803_01190_b200 import workloads
+
+
+def test_vertical_profile_is_the_sech2_sheet_when_rho_star_vanishes():
+    """eq. (4) with rho_* = 0 and <v_r v_z> = 0: rho = rho_0 sech^2(z/z_0), z_0 = c_z^2/(pi G Sigma), rho_0 = Sigma/2z_0."""
+    for G, Sigma, c_z in ((1.0, 0.17, 0.23), (2.5, 0.02, 0.05)):
+        z0 = c_z ** 2 / (math.pi * G * Sigma)
+        z, rho, rho0 = disk_ic.vertical_profile(Sigma, c_z, 0.0, G=G, z0_guess=z0)
+        assert abs(rho0 - Sigma / (2 * z0)) <= 1e-6 * rho0
+        ok = z <= 6 * z0
+        assert np.max(np.abs(rho[ok] - rho0 / np.cosh(z[ok] / z0) ** 2) / rho0) <= 1e-6
+        # a wrong guess of the scale height (it only sets the grid) gives the same profile
+        z2, rho2, rho02 = disk_ic.vertical_profile(Sigma, c_z, 0.0, G=G, z0_guess=1.5 * z0)
+        assert abs(rho02 - rho0) <= 1e-5 * rho0
+
+
+@pytest.mark.parametrize("rho_star_frac", [-0.3, 0.2])
+def test_vertical_profile_satisfies_eq4_and_the_column(rho_star_frac):
+    """rho rho'' - rho'^2 + (4 pi G rho^2 / c_z^2)(rho - rho_*) = 0 (eq. (4) as printed, <v_r v_z> = 0) by central
+    differences on the returned profile, and 2 int rho dz = Sigma."""
+    G, Sigma, c_z, z0 = 1.0, 0.1, 0.18, 0.1
+    rho_star = rho_star_frac * Sigma / (2 * z0)
+    z, rho, rho0 = disk_ic.vertical_profile(Sigma, c_z, rho_star, G=G, z0_guess=z0)
+    dz = z[1] - z[0]
+    col = dz * (rho.sum() - 0.5 * (rho[0] + rho[-1]))
+    # rho_* > 0: the solution has a minimum (rho never reaches 0) where the profile is cut; moving the cut by one grid
+    # step changes the column by rho_min dz, which bounds how well the bisection can match Sigma
+    assert abs(2 * col - Sigma) <= (1e-9 if rho_star <= 0 else 2 * rho.min(initial=1.0, where=rho > 0) * dz / Sigma * 2) * Sigma
+    i = np.arange(1, 150)                                  # z <= 3 z0
+    i = i[rho[i + 1] > 1e-6 * rho0]                        # rho well above round-off
+    # divided by rho^2 the first two terms are (ln rho)'' -- differenced in that form, which does not cancel
+    y = np.log(rho[:i[-1] + 2])
+    d2 = (y[i + 1] - 2 * y[i] + y[i - 1]) / dz ** 2
+    res = d2 + 4 * math.pi * G / c_z ** 2 * (rho[i] - rho_star)
+    scale = 4 * math.pi * G / c_z ** 2 * (rho[i] + abs(rho_star))
+    assert len(i) > 50 and np.max(np.abs(res) / scale) <= 1e-4      # O(dz^2) of the difference quotient
+    # a positive rho_* (rising rotation curve) thickens the layer, a negative one (falling) thins it
+    _, _, rho0_free = disk_ic.vertical_profile(Sigma, c_z, 0.0, G=G, z0_guess=z0)
+    assert (rho0 < rho0_free) == (rho_star > 0)
+
+
+def test_radius_inverts_the_exponential_disk_mass():
+    u = np.array([1e-6, 0.1, 0.5, 0.9, 1 - 1e-9])
+    R = disk_ic.radius_from_uniform(u, h=2.0)
+    assert np.allclose(workloads.disk_enclosed_mass(R, h=2.0), u, rtol=0, atol=1e-14)
+    Rs = disk_ic.radius_from_uniform(workloads.jeans_disk_draws(20000, 3)["u_R"])
+    mean = (2 - 26 * math.exp(-4)) / (1 - 5 * math.exp(-4))         # <R> of the truncated Gamma(2) law, SURVEY P10
+    assert abs(Rs.mean() - mean) <= 4 * 0.9 / math.sqrt(20000)
+
+
+@pytest.fixture(scope="module")
+def disk():
+    n = 8192
+    d = workloads.jeans_disk_draws(n, 7)
+    pos, vel, mass, info = disk_ic.jeans_disk(d, G=1.0, delta=0.02, nthreads=0)
+    return n, pos, vel, mass, info
+
+
+def test_generated_disk_satisfies_the_radial_jeans_balance(disk):
+    """eq. (3) with every term MEASURED from the particles: mean v_phi, the dispersions and the radial force per radial
+    bin (8 wide bins over 0.75 h .. 3.75 h, 300-1300 bodies each) -- the residual is sampling noise, O(N_bin^-1/2) of
+    V_c^2 (plus the variation of the profiles across a wide bin)."""
+    n, pos, vel, mass, info = disk
+    acc, _ = oracle.forces(pos, mass, G=1.0, delta=0.02, want_pot=False, nthreads=0)
+    R = np.hypot(pos[:, 0], pos[:, 1])
+    c, s = pos[:, 0] / R, pos[:, 1] / R
+    vR, vp = vel[:, 0] * c + vel[:, 1] * s, -vel[:, 0] * s + vel[:, 1] * c
+    g_r = -(acc[:, 0] * c + acc[:, 1] * s)
+    edges = np.linspace(0.75, 3.75, 9)
+    mid = 0.5 * (edges[1:] + edges[:-1])
+    lhs, rhs, cnt = [], [], []
+    for lo, hi in zip(edges[:-1], edges[1:]):
+        sel = (R >= lo) & (R < hi)
+        cr2, cp2 = vR[sel].var(), vp[sel].var()
+        grad = np.interp(0.5 * (lo + hi), info["R_bin"], info["dln_rho_cr2_dlnR"])
+        lhs.append(vp[sel].mean() ** 2)
+        rhs.append((R[sel] * g_r[sel]).mean() + cr2 * (1 - cp2 / cr2 + grad))
+        cnt.append(sel.sum())
+    lhs, rhs = np.array(lhs), np.array(rhs)
+    vc2 = np.interp(mid, info["R_bin"], info["Vc2"])
+    assert min(cnt) > 200
+    # (dropping the pressure term of eq. (3) would leave 0.1-0.3 of V_c^2 here; measured: <= 0.02, 0.05 in the first bin)
+    assert np.max(np.abs(lhs - rhs) / vc2) <= 0.06 and np.median(np.abs(lhs - rhs) / vc2) <= 0.025
+    # the asymmetric drift is real: the mean rotation is slower than circular where the disk is hot
+    assert np.all(lhs[:4] < vc2[:4])
+
+
+def test_cold_disk_rotates_at_the_circular_speed():
+    """c -> 0 (a very thin, very cold disk): eq. (3) reduces to v_phi^2 = r g_r, the textbook circular orbit."""
+    d = workloads.jeans_disk_draws(2048, 5)
+    pos, vel, mass, info = disk_ic.jeans_disk(d, delta=0.05, z0=1e-3, f_z=1.0, n_bins=16, nthreads=0)
+    assert np.max(info["c_r"]) < 0.03
+    sel = info["R_bin"] > 0.5
+    assert np.max(np.abs(info["vphi_mean"][sel] ** 2 / info["Vc2"][sel] - 1)) <= 0.02
+    acc, _ = oracle.forces(pos, mass, delta=0.05, want_pot=False, nthreads=0)
+    R = np.hypot(pos[:, 0], pos[:, 1])
+    vp = (-vel[:, 0] * pos[:, 1] + vel[:, 1] * pos[:, 0]) / R
+    g_r = -(acc[:, 0] * pos[:, 0] + acc[:, 1] * pos[:, 1]) / R
+    ring = (R > 1.0) & (R < 3.0)
+    assert abs(np.mean(vp[ring] ** 2) / np.mean(R[ring] * g_r[ring]) - 1) <= 0.03
+
+
+def test_generated_disk_is_in_virial_equilibrium(disk):
+    """2K/|W| = 1 for a stationary self-gravitating system; the configs' recipe (circular speed from a SPHERICAL mass
+    estimate, dispersion a fixed fraction of it) sits at 0.92 for the same N and softening."""
+    n, pos, vel, mass, info = disk
+    inv = oracle.invariants(pos, vel, mass, G=1.0, delta=0.02, nthreads=0)
+    q = -2 * inv["K"] / inv["W"]
+    c = workloads.config(0, N=n)
+    inv0 = oracle.invariants(c["pos"], c["vel"], c["mass"], G=1.0, delta=0.02, nthreads=0)
+    q0 = -2 * inv0["K"] / inv0["W"]
+    assert abs(q - 1) <= 0.03 and abs(q - 1) < 0.5 * abs(q0 - 1), (q, q0)
+    assert abs(np.mean(vel[:, 2] ** 2) / np.mean(np.interp(np.hypot(pos[:, 0], pos[:, 1]), info["R_bin"],
+                                                            info["c_z"]) ** 2) - 1) <= 0.05
