@@ -25,9 +25,10 @@ What the paper fixes, and the reading taken where it is garbled or silent (DESIG
       It is NOT the relaxation of refs [1, 15, 18]; it satisfies eqs. (3)-(4) for the profiles above up to O(N^-1/2).
   R16 (discretisation): n_bins equal-width radial bins on [0, R_max]; bin means; derivatives by central differences
       on the bin centres (one-sided at the ends; rho_* of the innermost bin from the solid-body form V_c^2 ~ R^2, i.e.
-      rho_* = Omega^2 / (2 pi G)); rho_* is capped at half the rho_* = 0 sheet's midplane density Sigma / (4 z_0) (eq. (4)
-      is a thin-disk equation; the cap only acts in the innermost, noisiest bins); profiles are interpolated linearly
-      in R to the particles.
+      rho_* = Omega^2 / (2 pi G)); rho_* is capped at 0.1 of the rho_* = 0 sheet's midplane density Sigma / (2 z_0):
+      eq. (4) is a thin-disk equation, and for rho_* comparable to rho no layer of the wanted column exists; the cap
+      only acts at R < 0.5 h, where the disk is not thin compared with R; profiles are interpolated linearly in R to
+      the particles.
 
 Random numbers are INPUTS (`draws`, from paper_1803_01190_b200.workloads.jeans_disk_draws): u_R, u_phi, u_z uniform in
 (0, 1), g[N,3] standard normal.
@@ -67,59 +68,62 @@ def radius_from_uniform(u, h=1.0):
 
 def _integrate_sheet(rho0, k, rho_star, dz, nz):
     """RK4 for y = ln rho:  y'' = -k (e^y - rho_star),  y(0) = ln rho0, y'(0) = 0, on z = 0, dz, ..., nz dz.
-    The profile ends where rho would start to rise again (y' >= 0 after the first step) or drops below 1e-30 rho0:
-    rho is 0 beyond.  Returns rho[nz + 1]."""
+    For rho_star > 0 the density has a minimum (y' returns to 0) where the layer ends: its height z_end is located by
+    linear interpolation of y' between the two grid points that bracket it, so that the column depends continuously on
+    rho0.  The layer also ends 69 e-folds below the midplane or at the end of the grid.
+    Returns (z[m+1], rho[m+1]): the grid points inside the layer plus the end point (z_end, rho_end)."""
     def f(y, p):
         return p, -k * (math.exp(y) - rho_star)
     y, p = math.log(rho0), 0.0
-    rho = np.zeros(nz + 1)
-    rho[0] = rho0
+    zs, rho = [0.0], [rho0]
     for n in range(nz):
         k1y, k1p = f(y, p)
         k2y, k2p = f(y + 0.5 * dz * k1y, p + 0.5 * dz * k1p)
         k3y, k3p = f(y + 0.5 * dz * k2y, p + 0.5 * dz * k2p)
         k4y, k4p = f(y + dz * k3y, p + dz * k3p)
-        y += dz * (k1y + 2 * k2y + 2 * k3y + k4y) / 6.0
-        p += dz * (k1p + 2 * k2p + 2 * k3p + k4p) / 6.0
-        if p >= 0.0 or y < math.log(rho0) - 69.0:
+        y_new = y + dz * (k1y + 2 * k2y + 2 * k3y + k4y) / 6.0
+        p_new = p + dz * (k1p + 2 * k2p + 2 * k3p + k4p) / 6.0
+        if p_new >= 0.0:                                   # the minimum lies in (z_n, z_n+1]
+            frac = p / (p - p_new) if n > 0 else 0.0
+            zs.append((n + frac) * dz)
+            rho.append(math.exp(y + frac * (y_new - y)))
             break
-        rho[n + 1] = math.exp(y)
-    return rho
+        if y_new < math.log(rho0) - 69.0:
+            break
+        y, p = y_new, p_new
+        zs.append((n + 1) * dz)
+        rho.append(math.exp(y))
+    return np.array(zs), np.array(rho)
+
+
+def _column(z, rho):
+    """int_0^z_end rho dz by the trapezoid rule on the (possibly uneven last) intervals."""
+    return float(np.sum(0.5 * (rho[1:] + rho[:-1]) * np.diff(z)))
 
 
 def vertical_profile(Sigma, c_z, rho_star, G=1.0, z0_guess=0.1, nz=600, zmax_over_z0=12.0):
-    """Solution of eq. (4) with <v_r v_z> = 0 for one radius: rho(z) on z = 0 .. zmax with the midplane density
-    chosen (bisection) so that 2 int_0^zmax rho dz = Sigma.  Returns (z[nz+1], rho[nz+1], rho0)."""
+    """Solution of eq. (4) with <v_r v_z> = 0 for one radius: rho(z) from the midplane to the end of the layer, with
+    the midplane density chosen (bisection) so that 2 int rho dz = Sigma.  Returns (z[m], rho[m], rho0)."""
     k = 4.0 * math.pi * G / (c_z * c_z)
-    zmax = zmax_over_z0 * z0_guess
-    dz = zmax / nz
-    z = dz * np.arange(nz + 1)
-
-    def column(rho0):
-        rho = _integrate_sheet(rho0, k, rho_star, dz, nz)
-        return dz * (rho.sum() - 0.5 * (rho[0] + rho[-1])), rho      # trapezoid
-
-    lo, hi = 1e-3 * Sigma / (2.0 * z0_guess), 1e3 * Sigma / (2.0 * z0_guess)
+    dz = zmax_over_z0 * z0_guess / nz
+    # For rho_* > 0 the column is not monotonic in rho0 (it diverges again as rho0 -> rho_*, where the layer becomes
+    # infinitely wide); the thin-disk solution is the branch rho0 >> rho_*, so the search starts at 2 rho_*.
+    lo, hi = max(1e-3 * Sigma / (2.0 * z0_guess), 2.0 * rho_star), 1e3 * Sigma / (2.0 * z0_guess)
     for _ in range(80):
         mid = math.sqrt(lo * hi)
-        col, _ = column(mid)
-        if 2.0 * col < Sigma:
+        if 2.0 * _column(*_integrate_sheet(mid, k, rho_star, dz, nz)) < Sigma:
             lo = mid
         else:
             hi = mid
     rho0 = math.sqrt(lo * hi)
-    _, rho = column(rho0)
+    z, rho = _integrate_sheet(rho0, k, rho_star, dz, nz)
     return z, rho, rho0
 
 
 def cumulative_column(z, rho):
-    """Normalised cumulative column int_0^z rho dz' / int_0^zmax rho dz' (trapezoid), up to the last z with rho > 0.
-    Returns (z_part, cum_part)."""
-    dz = z[1] - z[0]
-    cum = np.concatenate([[0.0], np.cumsum(0.5 * dz * (rho[1:] + rho[:-1]))])
-    cum /= cum[-1]
-    last = int(np.max(np.nonzero(rho > 0.0)[0]))
-    return z[:last + 1], cum[:last + 1]
+    """Normalised cumulative column int_0^z rho dz' / int_0^z_end rho dz' (trapezoid).  Returns (z, cum)."""
+    cum = np.concatenate([[0.0], np.cumsum(0.5 * (rho[1:] + rho[:-1]) * np.diff(z))])
+    return z, cum / cum[-1]
 
 
 def _z_from_uniform(u, z_part, cum_part):
@@ -169,7 +173,7 @@ def jeans_disk(draws, G=1.0, delta=0.02, h=1.0, M_d=1.0, z0=0.1, f_z=0.6, n_bins
     cz_b = np.sqrt(math.pi * G * Sigma_b * z0)                      # R14
     rho_star_b = dvc2 / (4.0 * math.pi * G * centres)               # eq. (4)
     rho_star_b[0] = vc2[0] / (2.0 * math.pi * G * centres[0] ** 2)  # innermost bin: solid-body rise V_c^2 ~ R^2 (R16)
-    rho_star_b = np.minimum(rho_star_b, 0.5 * Sigma_b / (2.0 * z0))   # thin-disk guard: rho_* <= half the sheet's rho_0
+    rho_star_b = np.minimum(rho_star_b, 0.1 * Sigma_b / (2.0 * z0))   # thin-disk guard: rho_* <= 0.1 of the sheet's rho_0
     # pass 2: eq. (4) with rho_* per bin; z re-placed from its cumulative column
     profiles = [vertical_profile(Sigma_b[b], cz_b[b], rho_star_b[b], G, z0) for b in range(n_bins)]
     columns = [cumulative_column(p[0], p[1]) for p in profiles]
