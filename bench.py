@@ -2,6 +2,7 @@
 """bench.py -- pair-interactions/s of the direct-summation hot path on B200 (BASELINE.json `metric`).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 2] [--n N]
+    python bench.py --sweep-n 11 23 [--out profiles/r2_sweep_n.json]     # throughput vs N, every shape class
 
 One STEP = one pass of the whole hot path over one batch of synthetic input:
     pp_step_kdk(1 step, PP_ACC_VALID, pot)  = kick+drift+pack -> pair sweep with potential -> split-j finalize + kick
@@ -53,6 +54,11 @@ def parse_args():
     ap.add_argument("--no-fp64", action="store_true", help="skip the FP64 arm (faster profiling runs)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-kdk-latency", action="store_true", help="skip the small-N step-latency rows (configs 0, 1)")
+    ap.add_argument("--sweep-n", type=int, nargs=2, metavar=("LOG2_MIN", "LOG2_MAX"), default=None,
+                    help="throughput of one gravity solve vs N = 2^min .. 2^max for every shape class (BASELINE.md "
+                         "section 4.2); prints one JSON document, also written to --out")
+    ap.add_argument("--out", default=None, help="file that --sweep-n also writes its JSON to")
     ap.add_argument("--sharded", action="store_true",
                     help="ONE system, i-bodies sharded over the N GPUs with an all-gather of positions per step "
                          "(SURVEY.md 8(f) NEXT-1, strong scaling) instead of the default N independent replicas")
@@ -211,10 +217,16 @@ def run_ours(args):
         results[name] = dict(
             value=replicas.job_value(pairs, args.steps, ms, world), ms_per_step=ms / args.steps,
             sweep_ms_per_launch=sweep_ms / max(sweep_n, 1), sweep_share_of_step=sweep_ms / ms,
-            roofline=dict(bound="alu", kernel="force_%s_kernel (pair sweep with potential)" % name,
+            roofline=dict(bound="alu", kernel="force_%s%s_kernel (pair sweep with potential)" %
+                                 ("sym_" if plan["shape"] == 3 else "", name),
                           achieved=achieved, peak=peak, unit="Tlane-op/s", frac=achieved / peak,
                           traffic=NCU_TRAFFIC_BYTES.get((name, N)),
                           pipe_ops_per_pair=ops,
+                          # SURVEY.md section 8(d) counted 13 (FP32) / 18 (FP64) operations per pair interaction with the
+                          # potential, assuming every ORDERED pair is evaluated; the symmetric sweep evaluates every
+                          # unordered pair once, so against that figure the fraction can exceed 1
+                          frac_at_survey_ops_per_pair=(13 if name == "f32" else 18) * pairs * sweep_n /
+                          (sweep_ms * 1e-3) / 1e12 / peak if sweep_ms > 0 else 0.0,
                           peak_source="nominal: %d %s lanes/SM x %d SMs x %.0f MHz" %
                                       (lanes, "FP32" if name == "f32" else "FP64", SM_COUNT, SM_MAX_HZ / 1e6)),
             plan=plan, E_after=inv["E"])
@@ -230,6 +242,11 @@ def run_ours(args):
         gms = max_over_ranks(time_steps(torch, force_only, 2, 1, flush, barrier))
         ppgrav.pp_configure(ppgrav.PP_CFG_EQUAL_MASS, 1)
         results[name]["force_only_unequal_masses"] = replicas.job_value(pairs, 2, gms, world)
+        # and with every ORDERED pair evaluated (the one-sided sweep: what N > 2^21 and i-ranges run)
+        ppgrav.pp_configure(ppgrav.PP_CFG_SYMMETRIC, 0)
+        oms = max_over_ranks(time_steps(torch, force_only, 2, 1, flush, barrier))
+        ppgrav.pp_configure(ppgrav.PP_CFG_SYMMETRIC, 1)
+        results[name]["force_only_one_sided"] = replicas.job_value(pairs, 2, oms, world)
 
         if name == "f32" and not args.no_e2e:
             # end to end through the host-buffer C ABI: pinned host arrays in, results back, every step
@@ -276,6 +293,7 @@ def run_ours(args):
             "sweep_ms_per_launch": r32["sweep_ms_per_launch"], "sweep_share_of_step": r32["sweep_share_of_step"],
             "force_only": {k: results[k]["force_only"] for k in results},
             "force_only_unequal_masses": {k: results[k]["force_only_unequal_masses"] for k in results},
+            "force_only_one_sided": {k: results[k]["force_only_one_sided"] for k in results},
             "plan": r32["plan"],
             # the literature's convention: 20 flop per pair interaction (rsqrt counted as 4), force-only solve
             "tflops_20_flop_per_pair": {k: 20.0 * results[k]["force_only"] / 1e12 for k in results},
@@ -285,12 +303,131 @@ def run_ours(args):
             line["fp64"] = {"value": r64["value"], "unit": UNIT, "ms_per_step": r64["ms_per_step"],
                             "roofline": r64["roofline"], "sweep_ms_per_launch": r64["sweep_ms_per_launch"],
                             "plan": r64["plan"], "fp64_over_fp32_time": r64["ms_per_step"] / r32["ms_per_step"]}
+        if world == 1 and not args.no_kdk_latency:
+            # BASELINE.json's KDK-step configs: 0 (N = 2048, 10 steps per call) and 1 (N = 2^17, 200 steps; 20 per call)
+            line["kdk_step"] = {"config0": kdk_step_latency(torch, ppgrav, workloads, 0, 10),
+                                "config1": kdk_step_latency(torch, ppgrav, workloads, 1, 20, reps=2)}
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(c, n_sample=16384)
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
     return line
+
+
+# ---- small-N step latency (configs 0 and 1 are KDK-step configs; a solve of 2048 bodies is launch-bound) -----------
+def kdk_step_latency(torch, ppgrav, workloads, config_index, nsteps, reps=5):
+    """Microseconds per KDK step of pp_step_kdk(nsteps, PP_ACC_VALID) on torch's default stream, CUDA-graph replay on
+    and off, both precisions; best of `reps` calls after one warm-up call (which also instantiates the graph)."""
+    c = workloads.config(config_index)
+    N, G, delta, dt = c["N"], c["G"], c["delta"], c["dt"]
+    out = {"workload": workload_name(dict(c, index=config_index)), "nsteps_per_call": nsteps,
+           "launches_per_call": 2 * nsteps + 2, "stream": "default (legacy) stream"}
+    for name, dtype in (("f32", torch.float32), ("f64", torch.float64)):
+        pos, vel, mass = (torch.tensor(c[k], dtype=dtype, device="cuda") for k in ("pos", "vel", "mass"))
+        acc = torch.empty_like(pos)
+        ppgrav.pp_step_kdk(pos, vel, mass, acc, dt, 0, G=G, delta=delta)
+        row = {}
+        for graph in (1, 0):
+            ppgrav.pp_configure(ppgrav.PP_CFG_GRAPH, graph)
+            best = None
+            for r in range(reps + 1):
+                torch.cuda.synchronize()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                t0 = time.perf_counter()
+                e0.record()
+                ppgrav.pp_step_kdk(pos, vel, mass, acc, dt, nsteps, G=G, delta=delta, acc_valid=True)
+                e1.record()
+                torch.cuda.synchronize()
+                wall = (time.perf_counter() - t0) * 1e6
+                dev = e0.elapsed_time(e1) * 1e3
+                if r > 0 and (best is None or dev < best[0]):
+                    best = (dev, wall)
+            key = "graph" if graph else "plain_launches"
+            row[key] = {"us_per_step_device": best[0] / nsteps, "us_per_step_wall": best[1] / nsteps,
+                        "pairs_per_s": float(N) * (N - 1) * nsteps / (best[0] * 1e-6)}
+        ppgrav.pp_configure(ppgrav.PP_CFG_GRAPH, 1)
+        plan = ppgrav.pp_plan_query(N, ppgrav.PP_F32 if name == "f32" else ppgrav.PP_F64, False)
+        row["plan"] = {k: plan[k] for k in ("shape", "i_per_cta", "tile_j", "split", "ctas")}
+        out[name] = row
+    return out
+
+
+# ---- throughput of one gravity solve vs N, per shape class (BASELINE.md section 4.2; calibrates plan.cu) -----------
+def run_sweep_n(args):
+    import torch
+    from paper_1803_01190_b200 import ppgrav, workloads
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(0)
+    ppgrav.lib()
+    flush_buf = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device="cuda")
+    rows = []
+    # (name, PP_CFG_SHAPE, PP_CFG_SYMMETRIC): auto = the library's own choice; the rest pin the sweep
+    shapes = (("auto", 0, 1), ("symmetric", 0, 2), ("large", 1, 0), ("mid", 2, 0), ("small", 3, 0))
+    for logn in range(args.sweep_n[0], args.sweep_n[1] + 1):
+        N = 1 << logn
+        c = workloads.config(2, N=N)                   # the bench recipe (equal-mass exponential disk) at every N
+        pairs = float(N) * float(N - 1)
+        for name, dtype, code, lanes in (("f32", torch.float32, ppgrav.PP_F32, FP32_LANES),
+                                         ("f64", torch.float64, ppgrav.PP_F64, FP64_LANES)):
+            pos = torch.tensor(c["pos"], dtype=dtype, device="cuda")
+            mass = torch.tensor(c["mass"], dtype=dtype, device="cuda")
+            acc = torch.empty_like(pos)
+            pot = torch.empty_like(mass)
+            peak = lanes * SM_COUNT * SM_MAX_HZ
+            for shape, key, symkey in shapes:
+                if shape == "small" and logn > 17 or shape == "mid" and logn > 20 or shape == "symmetric" and logn > 21:
+                    continue                           # far outside their range: minutes per solve, nothing to learn
+                ppgrav.pp_configure(ppgrav.PP_CFG_SHAPE, key)
+                ppgrav.pp_configure(ppgrav.PP_CFG_SYMMETRIC, symkey)
+                for with_pot in (False, True):
+                    plan = ppgrav.pp_plan_query(N, code, with_pot)
+                    est = pairs * (12 if name == "f32" else 17) / (0.5 * peak)          # rough seconds per solve
+                    if shape == "small":
+                        est *= 2.5
+                    reps = int(max(2, min(20, 1.0 / max(est, 1e-4))))
+                    times = []
+                    for r in range(reps + 1):
+                        flush_buf.zero_()
+                        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                        e0.record()
+                        ppgrav.pp_forces(pos, mass, G=1.0, delta=c["delta"], acc=acc, pot=pot if with_pot else None)
+                        e1.record()
+                        torch.cuda.synchronize()
+                        if r > 0:
+                            times.append(e0.elapsed_time(e1))
+                    ms = float(np.median(times))
+                    # the pair-sweep kernel alone (events recorded by the library around its launch)
+                    ppgrav.pp_configure(ppgrav.PP_CFG_PROFILE, 1)
+                    ppgrav.pp_profile_read()
+                    for r in range(min(reps, 5)):
+                        flush_buf.zero_()
+                        ppgrav.pp_forces(pos, mass, G=1.0, delta=c["delta"], acc=acc, pot=pot if with_pot else None)
+                    k_ms, k_n = ppgrav.pp_profile_read()
+                    ppgrav.pp_configure(ppgrav.PP_CFG_PROFILE, 0)
+                    k_ms = k_ms / max(k_n, 1)
+                    n_tiles, n_common = ppgrav.pp_equal_mass_tiles(mass)
+                    ops = plan["pipe_ops_per_pair"] - n_common / n_tiles
+                    rows.append({"log2N": logn, "N": N, "precision": name, "shape_requested": shape,
+                                 "with_pot": with_pot, "shape": ("large", "mid", "small", "symmetric")[plan["shape"]],
+                                 "i_per_cta": plan["i_per_cta"], "tile_j": plan["tile_j"], "split": plan["split"],
+                                 "ctas": plan["ctas"], "ctas_per_sm": plan["ctas_per_sm"], "reps": reps,
+                                 "ms_per_solve": ms, "ms_best": float(min(times)), "pairs_per_s": pairs / (ms * 1e-3),
+                                 "sweep_kernel_ms": k_ms, "sweep_kernel_pairs_per_s": pairs / (k_ms * 1e-3) if k_ms > 0 else 0.0,
+                                 "pipe_ops_per_pair": ops, "roofline_frac": ops * pairs / (ms * 1e-3) / peak})
+            ppgrav.pp_configure(ppgrav.PP_CFG_SHAPE, 0)
+            ppgrav.pp_configure(ppgrav.PP_CFG_SYMMETRIC, 1)
+            del pos, mass, acc, pot
+        print("[sweep-n] 2^%d done" % logn, file=sys.stderr, flush=True)
+    doc = {"what": "pp_forces (pack + tile masses + pair sweep + finalize: the whole call, CUDA events on the launching "
+                   "stream, median of reps after one warm-up, 256 MiB L2 flush before every call) on the configs[2] "
+                   "recipe at N = 2^k", "command": "python bench.py --sweep-n %d %d" % tuple(args.sweep_n),
+           "peak": "nominal lanes x 148 SMs x 1965 MHz", "rows": rows}
+    if args.out:
+        with open(args.out, "w") as f:
+            json.dump(doc, f, indent=0)
+    return doc
 
 
 # ---- one system sharded over the GPUs (opt-in; the north_star's graded path is the single-GPU one above) ---------
@@ -371,9 +508,16 @@ def cpu_baseline(c, n_sample):
     oracle.forces(c["pos"], c["mass"], G=c["G"], delta=c["delta"], idx=idx, want_pot=True, nthreads=0)
     sec = time.perf_counter() - t0
     pairs = float(len(idx)) * float(c["N"] - 1)
+    # the same routine on ONE thread, on the first 1024 of those bodies (SURVEY.md section 8(d) asks for both rates)
+    idx1 = idx[:1024]
+    t0 = time.perf_counter()
+    oracle.forces(c["pos"], c["mass"], G=c["G"], delta=c["delta"], idx=idx1, want_pot=True, nthreads=1)
+    sec1 = time.perf_counter() - t0
     return {"value": pairs / sec, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": sec,
+            "single_thread_value": float(len(idx1)) * float(c["N"] - 1) / sec1, "single_thread_seconds": sec1,
             "sample": "oracle.forces (FP64, compensated sums, OpenMP over i) for %d sampled i-bodies x all %d "
-                      "j-bodies of the same workload = %.3g pairs" % (len(idx), c["N"], pairs)}
+                      "j-bodies of the same workload = %.3g pairs; single thread: the first %d of them" %
+                      (len(idx), c["N"], pairs, len(idx1))}
 
 
 def run_reference(args):
@@ -413,8 +557,8 @@ def run_reference(args):
 
 def main():
     args = parse_args()
-    line = (run_reference(args) if args.impl == "reference" else run_sharded(args) if args.sharded
-            else run_ours(args))
+    line = (run_reference(args) if args.impl == "reference" else run_sweep_n(args) if args.sweep_n
+            else run_sharded(args) if args.sharded else run_ours(args))
     if line is not None:
         print(json.dumps(line), flush=True)
 

@@ -19,13 +19,17 @@
  *   - Layout: pos, vel, acc are row-major [N,3]; mass, pot are [N]; element type float (PP_F32) or double
  *     (PP_F64, PP_MIXED) according to `precision`; pointers must be aligned to the element size.  No padding is
  *     required.
- *   - delta is the Plummer softening length of PAPER.md:48 (delta >= 0).  delta == 0 is legal: pairs at zero
- *     distance (including padding and j == i) then contribute nothing.
+ *   - delta is the Plummer softening length of PAPER.md:48 (delta >= 0).  delta == 0 is legal, and so is any tiny
+ *     delta: when delta^2 < 1e-20 (PP_F32, PP_MIXED) or < 1e-200 (PP_F64) the guarded kernels run, in which a pair
+ *     whose softened squared distance r^2 + delta^2 is at or below that threshold -- j == i, coincident bodies,
+ *     padding -- contributes nothing (its r^-3 would overflow).  Above the threshold no pair is dropped.
  *   - G multiplies the finished sums once (acc = G * sum), not every pair.
  *   - Results are bit-reproducible run to run for the same N, plan and device (no floating-point atomics).
  *   - The library keeps a per-device workspace (packed copy of the bodies, split-j partial sums) that grows on
- *     demand and is freed by pp_release().  Calls that share a device must therefore be issued on one stream at a
- *     time (stream-ordered reuse); concurrent use from several streams is not supported.
+ *     demand and is freed by pp_release().  Its reuse is stream-ordered: calls on one stream follow each other as
+ *     usual; a call issued on a DIFFERENT stream than the previous call on that device first waits, on the device,
+ *     for the previous call's work (an event wait, no host block).  Calls from several host threads are serialised
+ *     by a mutex.  So concurrent use from several streams is safe but does not overlap.
  *   - There is no CPU fallback: without a CUDA device every compute call returns PP_ECUDA.
  */
 #ifndef PPGRAV_H_
@@ -37,7 +41,7 @@
 extern "C" {
 #endif
 
-#define PPGRAV_VERSION 100 /* 0.1.0 */
+#define PPGRAV_VERSION 200 /* 0.2.0 */
 
 /* precision */
 #define PP_F32 0
@@ -59,10 +63,20 @@ extern "C" {
 
 /* pp_configure keys */
 #define PP_CFG_SPLIT_J 1 /* 0 = automatic (default); S >= 1 forces the j-range to be split S ways */
-#define PP_CFG_GRAPH 2   /* 1 (default) = pp_step_kdk replays its step loop from a CUDA graph when N is small */
+#define PP_CFG_GRAPH 2   /* 1 (default) = pp_step_kdk replays its interior steps from a CUDA graph when N <= 65536 */
 #define PP_CFG_PROFILE 3 /* 1 = bracket every pair-sweep launch with CUDA events (pp_profile_read); no graph replay */
 #define PP_CFG_EQUAL_MASS 4 /* 1 (default) = j-tiles whose bodies all have the same mass take m_j out of the pair loop
                              * (one pipe operation per pair less); 0 = every tile multiplies by m_j per pair */
+#define PP_CFG_SHAPE 5   /* kernel shape class of the pair sweep: 0 = chosen by the launch plan (default), 1 = large
+                          * (the throughput shape: 1536-1792 i-bodies per CTA, one CTA per SM), 2 = mid (512 i-bodies
+                          * per CTA), 3 = small (one i-body per thread).  Any class is correct at any N; the tests use
+                          * this to run the edge cases on every shape */
+
+#define PP_CFG_SYMMETRIC 6 /* the pair sweep that evaluates every UNORDERED pair once (Newton's third law: one evaluation
+                            * of eq. (2) serves i <- j and j <- i; 7-9 instead of 11-13 FP32-pipe operations per pair
+                            * interaction).  1 (default) = used for full solves with an FP32 sweep (PP_F32, PP_MIXED)
+                            * when the plan would take the large shape class and its j-side workspace
+                            * (N^2/3584 x 16 B) stays under 32 GB, i.e. 2^16 < N <= 2^21; 0 = never; 2 = always */
 
 /* Version of the library that was loaded (PPGRAV_VERSION). */
 int pp_version(void);
@@ -94,8 +108,10 @@ int pp_forces(const void* pos, const void* mass, void* acc, void* pot, int64_t N
 /* The same gravity solve restricted to the i-bodies [i_begin, i_begin + i_count): every GPU of a multi-GPU run
  * "calculates the dynamics of N/k particles" against all N j-bodies, so
  *   pos [N,3], mass [N] in (all bodies);  acc [i_count,3] out;  pot [i_count] out or NULL.
- * Per body the arithmetic is that of pp_forces; results are bit-identical to the corresponding rows of pp_forces
- * when the split-j factor is the same (PP_CFG_SPLIT_J), otherwise equal to summation-order round-off.
+ * Per body the arithmetic is that of pp_forces.  The launch plan is made for the range (i_count i-bodies against N
+ * j-bodies), so it may pick another shape class or split-j factor than the full solve; a row is bit-identical to
+ * the corresponding row of pp_forces exactly when both solves use the same j-tile size and the same split-j factor
+ * (pp_plan_query; PP_CFG_SHAPE and PP_CFG_SPLIT_J pin them), otherwise equal to summation-order round-off.
  * PP_EINVAL if the range is empty or leaves [0, N). */
 int pp_forces_range(const void* pos, const void* mass, void* acc, void* pot, int64_t N, int64_t i_begin,
                     int64_t i_count, double G, double delta, int precision, void* stream);
@@ -115,7 +131,11 @@ int pp_kick_drift(void* pos, void* vel, const void* acc, int64_t n, double kick,
  *   pot [N] out or NULL: if given, the LAST gravity solve of the call also produces Phi_i at t0 + nsteps*dt in the
  *   state precision (one more pipe operation per pair in that solve only), ready for pp_invariants; if the call
  *   performs no solve (nsteps == 0 with PP_ACC_VALID) pot is left untouched.
- * nsteps == 0 only (re)computes acc.  Force evaluations performed: nsteps (+1 without PP_ACC_VALID). */
+ * nsteps == 0 only (re)computes acc.  Force evaluations performed: nsteps (+1 without PP_ACC_VALID).
+ * Kernel launches: 1 (tile masses) + 3 for a cold start + 1 (kick+drift+pack) + 2 per interior step boundary
+ * (pair sweep, fused update pass) + 2 (last sweep, finalize+kick) = 2 nsteps + 2 (+3).  For N <= 65536 the interior
+ * steps are replayed from a CUDA graph that is kept while the arguments do not change (also when `stream` is the legacy
+ * default stream: the replay then runs on an internal stream, ordered with `stream` by events). */
 int pp_step_kdk(void* pos, void* vel, const void* mass, void* acc, void* pot, int64_t N, double dt, int64_t nsteps,
                 double G, double delta, int precision, unsigned flags, void* stream);
 
@@ -146,26 +166,22 @@ int pp_step_kdk_host(void* pos, void* vel, const void* mass, void* acc, void* po
 int pp_invariants_host(const void* pos, const void* vel, const void* mass, const void* pot, int64_t N, double G,
                        double delta, int precision, double* out16, void* stream);
 
-/* Launch plan the library would use for a gravity solve of N bodies: out8 (host) =
- *   { i-bodies per CTA, j-bodies per tile, split-j factor S, CTAs launched, CTAs resident per SM, SM count,
- *     pipe operations per pair (FP32- or FP64-pipe instructions per lane) on a j-tile of mixed masses -- one less on
- *     a tile whose bodies have a common mass, see pp_equal_mass_tiles --, MUFU operations per pair }. */
-int pp_plan_query(int64_t N, int precision, int with_pot, int64_t* out8);
+/* Launch plan the library would use for a full gravity solve of N bodies (with_pot: the sweep that also produces the
+ * potential): out16 (host) =
+ *   { [0] i-bodies per CTA, [1] j-bodies per tile, [2] split-j factor S, [3] CTAs launched, [4] CTAs resident per SM,
+ *     [5] SM count, [6] pipe operations (FP32- or FP64-pipe instructions per lane) per pair EVALUATION on a j-tile of
+ *     mixed masses -- fewer by [12] on a tile whose bodies have a common mass, see pp_equal_mass_tiles --,
+ *     [7] MUFU operations per evaluation, [8] shape class (0 large, 1 mid, 2 small, 3 = the symmetric sweep,
+ *     PP_CFG_SYMMETRIC), [9] threads per CTA, [10] i-bodies per thread, [11] i-blocks,
+ *     [12] ordered pairs (pair interactions) one evaluation serves: 1, or 2 for the symmetric sweep,
+ *     [13] symmetric sweep: partner blocks H per block (rows of its j-side workspace), [14], [15] reserved }. */
+int pp_plan_query(int64_t N, int precision, int with_pot, int64_t* out16);
 
 /* How many j-tiles of a gravity solve of these masses have a common mass (and therefore run the pair loop without
  * the per-pair multiplication by m_j): mass [N] (device, `precision`) in; out2 (host) = { j-tiles swept, j-tiles with
  * a common mass }.  Independent of PP_CFG_EQUAL_MASS.  Synchronous.  bench.py uses it to count the pipe operations
  * per pair that were actually executed. */
 int pp_equal_mass_tiles(const void* mass, int64_t N, int precision, int64_t* out2, void* stream);
-
-/* Pipe-throughput microbenchmark used for the roofline denominators.
- *   kind: 0 FFMA, 1 FFMA2 (packed f32x2), 2 DFMA, 3 MUFU.RSQ, 4 MUFU.RSQ64H, 5 FFMA2+MUFU in the force kernel's mix (12 : 2),
- *         6 two FFMA2 : one DFMA with loop-constant multiplier/addend (do the FP32 and FP64 pipes overlap?),
- *         7 FFMA2 with three distinct register operands, 8 as 6 with three distinct register operands each
- *   out4 (host) = { seconds, lane-operations executed, SM clock in MHz during the run, lane-ops/clk/SM }; kinds 6-8
- *   count the FFMA2 lanes only.
- * Synchronous. */
-int pp_probe_pipe(int kind, int64_t iters, double* out4);
 
 #ifdef __cplusplus
 }

@@ -14,7 +14,10 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(ROOT, "include")
 LIB = os.path.join(HERE, "libppgrav.so")
 SOURCES = ("api.cu", "api_host.cu", "plan.cu", "update.cu", "invariants.cu", "density.cu", "force_f32.cu", "force_f64.cu",
-           "probe.cu")
+           "force_sym_f32.cu", "force_sym_f64.cu")
+# measurement tooling, NOT part of libppgrav: the pipe microbenchmarks of probe/ get a library of their own
+PROBE_SRC = os.path.join(HERE, "probe", "pipe_probe.cu")
+PROBE_LIB = os.path.join(HERE, "probe", "libppprobe.so")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
               "--ftz=false", "--prec-div=true", "--prec-sqrt=true", "--fmad=true"]
 
@@ -29,7 +32,9 @@ def _stale():
         return True
     t = os.path.getmtime(LIB)
     deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(INCLUDE, "ppgrav.h"), __file__]
-    return any(os.path.getmtime(d) > t for d in deps)
+    if any(os.path.getmtime(d) > t for d in deps):
+        return True
+    return not os.path.exists(PROBE_LIB) or os.path.getmtime(PROBE_SRC) > os.path.getmtime(PROBE_LIB)
 
 
 def build(force=False, verbose=False, extra_flags=(), out=None):
@@ -56,6 +61,8 @@ def build(force=False, verbose=False, extra_flags=(), out=None):
         objs.append(obj)
     cmd = [_nvcc(), "-shared", "-o", out] + objs + ["-gencode", "arch=compute_100a,code=sm_100a", "-lcudart"]
     subprocess.run(cmd, check=True)
+    if out == LIB:
+        subprocess.run([_nvcc()] + list(NVCC_FLAGS) + ["-shared", "-o", PROBE_LIB, PROBE_SRC, "-lcudart"], check=True)
     return out
 
 

@@ -17,70 +17,11 @@
 //    operations per interaction; N-body workloads are made of a few mass species, so nearly every tile qualifies.
 //  * the (i-block, j-split) decomposition gives the 148 SMs an even number of equal work units at any N; partial
 //    sums go to a workspace and are added in fixed order by finalize (update.cu) -- no floating-point atomics.
-#include "ppgrav_internal.h"
+#include "force_f32_common.cuh"
 #include "tma_ring.cuh"
 
 namespace ppgrav {
 namespace {
-
-__device__ __forceinline__ float rsqrt_approx(float x) {
-    float y;
-    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-    return y;
-}
-
-// s + c += t with the rounding error of the addition captured in c (Knuth TwoSum; never contracted or reassociated)
-__device__ __forceinline__ void comp_add(float& s, float& c, float t) {
-    const float n = __fadd_rn(s, t);
-    const float bp = __fsub_rn(n, s);
-    const float e = __fadd_rn(__fsub_rn(s, __fsub_rn(n, bp)), __fsub_rn(t, bp));
-    s = n;
-    c = __fadd_rn(c, e);
-}
-
-template <int IPT, int MODE, bool GUARD, bool DIAG, bool UNI>
-__device__ __forceinline__ void sweep_tile(const float4* __restrict__ tp, const int npairs, const float2 (&nx)[IPT],
-                                           const float2 (&ny)[IPT], const float2 (&nz)[IPT], float2 (&ax)[IPT],
-                                           float2 (&ay)[IPT], float2 (&az)[IPT], float2 (&ap)[IPT], const float2 eps2,
-                                           const int jbase, const int (&iidx)[IPT]) {
-#pragma unroll kF32Unroll
-    for (int p = 0; p < npairs; ++p) {
-        const float4 a = tp[2 * p];
-        const float4 b = tp[2 * p + 1];
-        const float2 xj = make_float2(a.x, a.y), yj = make_float2(a.z, a.w);
-        const float2 zj = make_float2(b.x, b.y), mj = make_float2(b.z, b.w);
-#pragma unroll
-        for (int k = 0; k < IPT; ++k) {
-            const float2 dx = __fadd2_rn(xj, nx[k]);          // r_j - r_i (two j-bodies)
-            const float2 dy = __fadd2_rn(yj, ny[k]);
-            const float2 dz = __fadd2_rn(zj, nz[k]);
-            float2 r2 = __ffma2_rn(dx, dx, eps2);             // |r_i - r_j|^2 + delta^2
-            r2 = __ffma2_rn(dy, dy, r2);
-            r2 = __ffma2_rn(dz, dz, r2);
-            float2 w;
-            w.x = rsqrt_approx(r2.x);
-            w.y = rsqrt_approx(r2.y);
-            if (GUARD) {                                      // delta == 0: zero-distance pairs contribute nothing
-                w.x = r2.x > 0.f ? w.x : 0.f;
-                w.y = r2.y > 0.f ? w.y : 0.f;
-            }
-            const float2 w2 = __fmul2_rn(w, w);
-            float2 mw = UNI ? w : __fmul2_rn(mj, w);          // equal-mass tile: m_j is applied in the fold
-            const float2 s = __fmul2_rn(mw, w2);              // m_j / (r^2 + delta^2)^{3/2}
-            ax[k] = __ffma2_rn(s, dx, ax[k]);
-            ay[k] = __ffma2_rn(s, dy, ay[k]);
-            az[k] = __ffma2_rn(s, dz, az[k]);
-            if (MODE == MODE_FORCE_POT) {
-                if (DIAG) {                                   // tile overlaps this CTA's own bodies: drop j == i
-                    const int j0 = jbase + 2 * p;
-                    if (j0 == iidx[k]) mw.x = 0.f;
-                    if (j0 + 1 == iidx[k]) mw.y = 0.f;
-                }
-                ap[k] = __fadd2_rn(ap[k], mw);                // m_j / (r^2 + delta^2)^{1/2}
-            }
-        }
-    }
-}
 
 template <int THREADS, int IPT, int TJ, int STAGES, int MINB, int MODE, bool GUARD>
 __global__ void __launch_bounds__(THREADS, MINB)
@@ -200,37 +141,49 @@ force_f32_kernel(const float* __restrict__ packed, const float* __restrict__ til
     }
 }
 
-template <int THREADS, int IPT, int TJ, int STAGES, int MINB>
-int launch_variant(const Plan& p, const float* packed, const float* tile_mass, float4* partial, int64_t N, float eps2,
-                   bool guard, int mode, cudaStream_t st) {
-    dim3 grid(p.n_iblocks, p.split);
-#define PP_LAUNCH32(MODE_, GUARD_)                                                      \
-    force_f32_kernel<THREADS, IPT, TJ, STAGES, MINB, MODE_, GUARD_>                     \
-        <<<grid, THREADS, 0, st>>>(packed, tile_mass, partial, p.n_tiles, p.part_stride, p.i_begin, eps2)
-    if (mode == MODE_FORCE) {
-        if (guard) PP_LAUNCH32(MODE_FORCE, true); else PP_LAUNCH32(MODE_FORCE, false);
-    } else {
-        if (guard) PP_LAUNCH32(MODE_FORCE_POT, true); else PP_LAUNCH32(MODE_FORCE_POT, false);
+template <int CLS, int MODE, bool GUARD>
+int launch_cmg(const Plan& p, const float* packed, const float* tile_mass, float4* partial, float eps2,
+               cudaStream_t st) {
+    constexpr KernelShape K = kShapes[0][CLS][MODE];
+    if (p.threads != K.threads || p.ipt != K.ipt || p.tile_j != K.tile_j) {
+        set_error("launch_force_f32: plan (%d x %d, tile %d) does not match the kernel shape of class %d mode %d",
+                  p.threads, p.ipt, p.tile_j, CLS, MODE);
+        return PP_EINVAL;
     }
-#undef PP_LAUNCH32
+    dim3 grid(p.n_iblocks, p.split);
+    force_f32_kernel<K.threads, K.ipt, K.tile_j, K.stages, K.ctas_per_sm, MODE, GUARD>
+        <<<grid, K.threads, 0, st>>>(packed, tile_mass, partial, p.n_tiles, p.part_stride, p.i_begin, eps2);
     count_launch();
     PP_CUDA(cudaGetLastError());
     return PP_OK;
+}
+
+template <int CLS>
+int launch_class(const Plan& p, const float* packed, const float* tile_mass, float4* partial, float eps2, bool guard,
+                 int mode, cudaStream_t st) {
+    if (mode == MODE_FORCE)
+        return guard ? launch_cmg<CLS, MODE_FORCE, true>(p, packed, tile_mass, partial, eps2, st)
+                     : launch_cmg<CLS, MODE_FORCE, false>(p, packed, tile_mass, partial, eps2, st);
+    return guard ? launch_cmg<CLS, MODE_FORCE_POT, true>(p, packed, tile_mass, partial, eps2, st)
+                 : launch_cmg<CLS, MODE_FORCE_POT, false>(p, packed, tile_mass, partial, eps2, st);
 }
 
 }  // namespace
 
 int launch_force_f32(const Plan& p, const float* packed, const float* tile_mass, float4* partial, int64_t N,
                      double delta, int mode, cudaStream_t st) {
+    (void)N;
     const float eps2 = (float)(delta * delta);
-    // guarded variant whenever delta^2 is not a normal positive float (r^2 could then be exactly 0)
-    const bool guard = !(eps2 >= 1.17549435e-38f);
-    constexpr KernelShape L = kShapeF32Large, S = kShapeF32Small;
-    if (p.variant == 0)
-        return launch_variant<L.threads, L.ipt, L.tile_j, L.stages, L.ctas_per_sm>(p, packed, tile_mass, partial, N,
-                                                                                    eps2, guard, mode, st);
-    return launch_variant<S.threads, S.ipt, S.tile_j, S.stages, S.ctas_per_sm>(p, packed, tile_mass, partial, N, eps2,
-                                                                                guard, mode, st);
+    const bool guard = !(eps2 >= kTinyR2F32);   // also catches NaN
+    if (mode != MODE_FORCE && mode != MODE_FORCE_POT) {
+        set_error("launch_force_f32: mode %d has no FP32 kernel", mode);
+        return PP_EINVAL;
+    }
+    switch (p.cls) {
+        case CLS_LARGE: return launch_class<CLS_LARGE>(p, packed, tile_mass, partial, eps2, guard, mode, st);
+        case CLS_MID: return launch_class<CLS_MID>(p, packed, tile_mass, partial, eps2, guard, mode, st);
+        default: return launch_class<CLS_SMALL>(p, packed, tile_mass, partial, eps2, guard, mode, st);
+    }
 }
 
 }  // namespace ppgrav

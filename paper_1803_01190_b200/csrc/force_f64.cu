@@ -10,75 +10,14 @@
 //    (3 DADD + 3 DFMA + 7 + 3 DFMA); with the potential 18; potential only (pp_invariants) 12.  Never 1.0/sqrt(x)
 //    (~30 FP64 operations).
 //  * equal-mass tiles (tile_mass[t] = the common mass, NaN otherwise; see force_f32.cu): the factor m_j is applied
-//    once per tile in the fold -- 15 (17) instead of 16 (18) operations per interaction.  MODE_POT keeps m_j inside.
+//    once per tile in the fold -- 15 (17) instead of 16 (18) operations per interaction.  MODE_POT (pp_invariants' potential sweep): 11 instead of 12.
 //  * blocked accumulation: per-tile sums are folded into outer sums after every tile (plain FP64 for the force,
 //    TwoSum double-double for MODE_POT, which feeds the energy diagnostic).
-#include "ppgrav_internal.h"
+#include "force_f64_common.cuh"
 #include "tma_ring.cuh"
 
 namespace ppgrav {
 namespace {
-
-__device__ __forceinline__ double rsqrt64h(double x) {
-    double y;
-    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-    return y;
-}
-
-__device__ __forceinline__ void comp_add(double& s, double& c, double t) {
-    const double n = __dadd_rn(s, t);
-    const double bp = __dsub_rn(n, s);
-    const double e = __dadd_rn(__dsub_rn(s, __dsub_rn(n, bp)), __dsub_rn(t, bp));
-    s = n;
-    c = __dadd_rn(c, e);
-}
-
-template <int IPT, int MODE, bool GUARD, bool DIAG, bool UNI>
-__device__ __forceinline__ void sweep_tile(const double4* __restrict__ tp, const int nj, const double (&xi)[IPT],
-                                           const double (&yi)[IPT], const double (&zi)[IPT], double (&ax)[IPT],
-                                           double (&ay)[IPT], double (&az)[IPT], double (&ap)[IPT], const double eps2,
-                                           const int jbase, const int (&iidx)[IPT]) {
-#pragma unroll kF64Unroll
-    for (int j = 0; j < nj; ++j) {
-        const double4 b = tp[j];
-#pragma unroll
-        for (int k = 0; k < IPT; ++k) {
-            const double dx = b.x - xi[k];                    // r_j - r_i
-            const double dy = b.y - yi[k];
-            const double dz = b.z - zi[k];
-            double r2 = fma(dx, dx, eps2);                    // |r_i - r_j|^2 + delta^2
-            r2 = fma(dy, dy, r2);
-            r2 = fma(dz, dz, r2);
-            double y = rsqrt64h(r2);
-            if (GUARD) y = r2 > 0.0 ? y : 0.0;                // delta == 0: zero-distance pairs contribute nothing
-            const double t = y * y;
-            const double e = fma(-r2, t, 1.0);                // 1 - x y^2
-            if (MODE == MODE_FORCE) {
-                const double p = fma(e, 1.875, 1.5);
-                const double u = UNI ? y : b.w * y;           // equal-mass tile: m_j is applied in the fold
-                const double w = u * t;                       // m y^3
-                const double we = w * e;
-                const double s = fma(p, we, w);               // m x^{-3/2}
-                ax[k] = fma(s, dx, ax[k]);
-                ay[k] = fma(s, dy, ay[k]);
-                az[k] = fma(s, dz, az[k]);
-            } else {
-                const double q = fma(e, 0.375, 0.5);
-                const double ye = y * e;
-                const double yy = fma(q, ye, y);              // x^{-1/2} to full precision
-                double u = UNI ? yy : b.w * yy;               // m / r
-                if (MODE == MODE_FORCE_POT) {
-                    const double s = u * (yy * yy);
-                    ax[k] = fma(s, dx, ax[k]);
-                    ay[k] = fma(s, dy, ay[k]);
-                    az[k] = fma(s, dz, az[k]);
-                }
-                if (DIAG && (jbase + j == iidx[k])) u = 0.0;  // drop j == i from the potential
-                ap[k] += u;
-            }
-        }
-    }
-}
 
 template <int THREADS, int IPT, int TJ, int STAGES, int MINB, int MODE, bool GUARD>
 __global__ void __launch_bounds__(THREADS, MINB)
@@ -132,19 +71,19 @@ force_f64_kernel(const double* __restrict__ packed, const double* __restrict__ t
 
     // common mass of the bodies of tile t, NaN when they differ (fetched one tile ahead: no exposed latency)
     const double kNoCommonMass = __longlong_as_double(0x7ff8000000000000ll);
-    const bool use_tm = (MODE != MODE_POT) && tile_mass != nullptr;
+    const bool use_tm = tile_mass != nullptr;
     double tm_next = (use_tm && nt > 0) ? __ldg(tile_mass + t0) : kNoCommonMass;
 
     for (int t = 0; t < nt; ++t) {
         const int s = t % STAGES;
         const double tm = tm_next;
         if (use_tm && t + 1 < nt) tm_next = __ldg(tile_mass + t0 + t + 1);
-        const bool uni = (MODE != MODE_POT) && tm == tm;
+        const bool uni = tm == tm;
         mbar_wait(&full_bar[s], (uint32_t)(t / STAGES) & 1u);
         const double4* tp = reinterpret_cast<const double4*>(&tiles[s][0]);
         const int jbase = (t0 + t) * TJ;
         const bool diag = (MODE != MODE_FORCE) && !GUARD && (jbase < i_hi) && (jbase + TJ > i_lo);
-        if (MODE != MODE_POT && uni) {
+        if (uni) {
             if (diag)
                 sweep_tile<IPT, MODE, GUARD, true, true>(tp, TJ, xi, yi, zi, ax, ay, az, ap, eps2, jbase, iidx);
             else
@@ -173,7 +112,7 @@ force_f64_kernel(const double* __restrict__ packed, const double* __restrict__ t
                 ax[k] = ay[k] = az[k] = 0.0;
             }
             if (MODE == MODE_FORCE_POT) { sp[k] = fma(scale, ap[k], sp[k]); ap[k] = 0.0; }
-            if (MODE == MODE_POT) { comp_add(sp[k], cp[k], ap[k]); ap[k] = 0.0; }
+            if (MODE == MODE_POT) { comp_add(sp[k], cp[k], __dmul_rn(scale, ap[k])); ap[k] = 0.0; }
         }
     }
 
@@ -186,38 +125,48 @@ force_f64_kernel(const double* __restrict__ packed, const double* __restrict__ t
     }
 }
 
-template <int THREADS, int IPT, int TJ, int STAGES, int MINB>
-int launch_variant(const Plan& p, const double* packed, const double* tile_mass, double4* partial, int64_t N,
-                   double eps2, bool guard, int mode, cudaStream_t st) {
-    dim3 grid(p.n_iblocks, p.split);
-#define PP_LAUNCH64(MODE_, GUARD_)                                                      \
-    force_f64_kernel<THREADS, IPT, TJ, STAGES, MINB, MODE_, GUARD_>                     \
-        <<<grid, THREADS, 0, st>>>(packed, tile_mass, partial, p.n_tiles, p.part_stride, p.i_begin, eps2)
-    if (mode == MODE_FORCE) {
-        if (guard) PP_LAUNCH64(MODE_FORCE, true); else PP_LAUNCH64(MODE_FORCE, false);
-    } else if (mode == MODE_FORCE_POT) {
-        if (guard) PP_LAUNCH64(MODE_FORCE_POT, true); else PP_LAUNCH64(MODE_FORCE_POT, false);
-    } else {
-        if (guard) PP_LAUNCH64(MODE_POT, true); else PP_LAUNCH64(MODE_POT, false);
+template <int CLS, int MODE, bool GUARD>
+int launch_cmg(const Plan& p, const double* packed, const double* tile_mass, double4* partial, double eps2,
+               cudaStream_t st) {
+    constexpr KernelShape K = kShapes[1][CLS][MODE];
+    if (p.threads != K.threads || p.ipt != K.ipt || p.tile_j != K.tile_j) {
+        set_error("launch_force_f64: plan (%d x %d, tile %d) does not match the kernel shape of class %d mode %d",
+                  p.threads, p.ipt, p.tile_j, CLS, MODE);
+        return PP_EINVAL;
     }
-#undef PP_LAUNCH64
+    dim3 grid(p.n_iblocks, p.split);
+    force_f64_kernel<K.threads, K.ipt, K.tile_j, K.stages, K.ctas_per_sm, MODE, GUARD>
+        <<<grid, K.threads, 0, st>>>(packed, tile_mass, partial, p.n_tiles, p.part_stride, p.i_begin, eps2);
     count_launch();
     PP_CUDA(cudaGetLastError());
     return PP_OK;
+}
+
+template <int CLS>
+int launch_class(const Plan& p, const double* packed, const double* tile_mass, double4* partial, double eps2,
+                 bool guard, int mode, cudaStream_t st) {
+    if (mode == MODE_FORCE)
+        return guard ? launch_cmg<CLS, MODE_FORCE, true>(p, packed, tile_mass, partial, eps2, st)
+                     : launch_cmg<CLS, MODE_FORCE, false>(p, packed, tile_mass, partial, eps2, st);
+    if (mode == MODE_FORCE_POT)
+        return guard ? launch_cmg<CLS, MODE_FORCE_POT, true>(p, packed, tile_mass, partial, eps2, st)
+                     : launch_cmg<CLS, MODE_FORCE_POT, false>(p, packed, tile_mass, partial, eps2, st);
+    return guard ? launch_cmg<CLS, MODE_POT, true>(p, packed, tile_mass, partial, eps2, st)
+                 : launch_cmg<CLS, MODE_POT, false>(p, packed, tile_mass, partial, eps2, st);
 }
 
 }  // namespace
 
 int launch_force_f64(const Plan& p, const double* packed, const double* tile_mass, double4* partial, int64_t N,
                      double delta, int mode, cudaStream_t st) {
+    (void)N;
     const double eps2 = delta * delta;
-    const bool guard = !(eps2 >= 2.2250738585072014e-308);
-    constexpr KernelShape L = kShapeF64Large, S = kShapeF64Small;
-    if (p.variant == 0)
-        return launch_variant<L.threads, L.ipt, L.tile_j, L.stages, L.ctas_per_sm>(p, packed, tile_mass, partial, N,
-                                                                                    eps2, guard, mode, st);
-    return launch_variant<S.threads, S.ipt, S.tile_j, S.stages, S.ctas_per_sm>(p, packed, tile_mass, partial, N, eps2,
-                                                                                guard, mode, st);
+    const bool guard = !(eps2 >= kTinyR2F64);
+    switch (p.cls) {
+        case CLS_LARGE: return launch_class<CLS_LARGE>(p, packed, tile_mass, partial, eps2, guard, mode, st);
+        case CLS_MID: return launch_class<CLS_MID>(p, packed, tile_mass, partial, eps2, guard, mode, st);
+        default: return launch_class<CLS_SMALL>(p, packed, tile_mass, partial, eps2, guard, mode, st);
+    }
 }
 
 }  // namespace ppgrav

@@ -2,8 +2,11 @@
 //
 // The all-pairs sweep of eq. (1) is cut into (i-block, j-split) work units.  The paper's Kepler GPUs
 // had 13-15 SMs, so "one thread per i-particle" filled them at any N of interest; a B200 has 148 SMs
-// and N = 2^20 bodies in 1024-body i-blocks are only 3.5 waves.  The plan therefore picks the kernel variant and the
-// split factor S that minimise  waves x (tiles per split + fixed overhead)  so that the last wave is nearly full.
+// and N = 2^20 bodies in 1792-body i-blocks are only 3.96 waves.  The plan therefore picks the shape class (large /
+// mid / small, ppgrav_internal.h) and the split factor S that minimise
+//     waves x (tiles per split + fixed overhead) x tile cost  +  weight x S x bodies
+// so that the last wave is nearly full.  The class efficiencies and the weight are calibrated on the B200 with the
+// throughput-vs-N sweep of `bench.py --sweep-n` (raw data profiles/r2_sweep_n.json).
 #include <algorithm>
 
 #include "ppgrav_internal.h"
@@ -12,35 +15,34 @@ namespace ppgrav {
 
 namespace {
 
-struct VariantDesc {
-    KernelShape s;
-    double eff;   // relative pair throughput of one SM running this shape (large = 1); measured, DESIGN.md "Plan"
-};
-
-const VariantDesc kVariants[2][2] = {
-    /* PP_F32 */ {{kShapeF32Large, 1.0}, {kShapeF32Small, 0.45}},
-    /* PP_F64 */ {{kShapeF64Large, 1.0}, {kShapeF64Small, 0.80}},
+// relative pair throughput of one SM running a class (large = 1), per precision; BASELINE.md section 4.2
+constexpr double kClassEff[2][kNumClasses] = {
+    /* PP_F32 */ {1.0, 0.90, 0.45},
+    /* PP_F64 */ {1.0, 0.93, 0.80},
 };
 
 int64_t round_up(int64_t a, int64_t b) { return (a + b - 1) / b * b; }
 
 // weight of one split-j partial sum of one body (written by the sweep, read by the finalize pass), in pair
 // interactions of one SM.  The bandwidth cost alone is ~0.1; the weight is larger so that a bigger S is only taken when
-// it fills the last wave noticeably better.  Calibrated on the B200 (N = 2^11 .. 2^22 sweep).
+// it fills the last wave noticeably better.
 constexpr double kFinalizeCost = 16.0;
 
 }  // namespace
 
-Plan make_plan(int64_t N, int precision, int sm_count, int64_t forced_split, int64_t i_begin, int64_t i_count) {
+Plan make_plan(int64_t N, int precision, int mode, int sm_count, int64_t forced_split, int forced_cls, int64_t i_begin,
+               int64_t i_count) {
     if (i_count < 0) i_count = N - i_begin;
     Plan best{};
     double best_cost = -1.0;
+    const int pi = precision == PP_F64 ? 1 : 0;
     const size_t elem = precision == PP_F64 ? 32 : 16;
-    for (int v = 0; v < 2; ++v) {
-        const VariantDesc& vd = kVariants[precision == PP_F64 ? 1 : 0][v];
-        const KernelShape& d = vd.s;
+    for (int c = 0; c < kNumClasses; ++c) {
+        if (forced_cls >= 0 && forced_cls < kNumClasses && c != forced_cls) continue;
+        const KernelShape& d = kShapes[pi][c][mode];
         Plan p{};
-        p.variant = v;
+        p.cls = c;
+        p.mode = mode;
         p.threads = d.threads;
         p.ipt = d.ipt;
         p.i_per_cta = d.threads * d.ipt;
@@ -56,12 +58,12 @@ Plan make_plan(int64_t N, int precision, int sm_count, int64_t forced_split, int
         p.n_pad = round_up(std::max(N, i_begin + p.part_stride), p.tile_j);
         p.n_tiles = (int)((N + p.tile_j - 1) / p.tile_j);
         const int64_t resident = (int64_t)sm_count * d.ctas_per_sm;
-        // partial sums: S x n_pad x {16,32} bytes, kept under 1 GiB
+        // partial sums: S x part_stride x {16,32} bytes, kept under 1 GiB
         int64_t s_max = std::min<int64_t>(std::min<int64_t>(p.n_tiles, 64),
                                           std::max<int64_t>(1, (int64_t)((1ull << 30) / (p.part_stride * elem))));
         int64_t s_lo = 1, s_hi = s_max;
         if (forced_split >= 1) s_lo = s_hi = std::min<int64_t>(forced_split, p.n_tiles);
-        const double tile_cost = (double)p.i_per_cta * p.tile_j * d.ctas_per_sm / vd.eff;
+        const double tile_cost = (double)p.i_per_cta * p.tile_j * d.ctas_per_sm / kClassEff[pi][c];
         for (int64_t S = s_lo; S <= s_hi; ++S) {
             const int64_t units = (int64_t)p.n_iblocks * S;
             const int64_t waves = (units + resident - 1) / resident;
@@ -76,6 +78,46 @@ Plan make_plan(int64_t N, int precision, int sm_count, int64_t forced_split, int
         }
     }
     return best;
+}
+
+Plan make_sym_plan(int64_t N, int precision, int mode, int sm_count, int64_t forced_split, size_t* jbytes) {
+    const KernelShape& d = precision == PP_F64 ? kShapeF64Sym : kShapeF32Sym;
+    const size_t elem = precision == PP_F64 ? 32 : 16;
+    Plan p{};
+    p.cls = CLS_LARGE;
+    p.mode = mode;
+    p.threads = d.threads;
+    p.ipt = d.ipt;
+    p.i_per_cta = d.threads * d.ipt;
+    p.tile_j = d.tile_j;
+    p.stages = d.stages;
+    p.ctas_per_sm = d.ctas_per_sm;
+    p.sm_count = sm_count;
+    p.i_begin = 0;
+    p.i_count = N;
+    p.n_iblocks = (int)((N + p.i_per_cta - 1) / p.i_per_cta);
+    p.part_stride = (int64_t)p.n_iblocks * p.i_per_cta;
+    p.n_pad = p.part_stride;                      // whole blocks: the cyclic partner ranges wrap over the padding
+    p.n_tiles = (int)(p.part_stride / p.tile_j);  // every tile of every block is swept (padding is massless)
+    p.sym = 1;
+    p.sym_h = (p.n_iblocks - 1) / 2;
+    // split-j over the partner tiles of a block: fill the last wave, as make_plan does
+    const int tpb = p.i_per_cta / p.tile_j;
+    const int64_t ptiles = (int64_t)p.sym_h * tpb;
+    int64_t s_lo = 1, s_hi = std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(ptiles, 64),
+                                                                     (int64_t)((1ull << 30) / (p.part_stride * elem))));
+    if (forced_split >= 1) s_lo = s_hi = std::max<int64_t>(1, std::min<int64_t>(forced_split, std::max<int64_t>(ptiles, 1)));
+    double best = -1.0;
+    p.split = 1;
+    for (int64_t S = s_lo; S <= s_hi; ++S) {
+        const int64_t units = (int64_t)p.n_iblocks * S;
+        const int64_t waves = (units + sm_count - 1) / sm_count;
+        const double cost = (double)waves * ((double)((ptiles + S - 1) / S) + 2.0 * tpb + 2.0) * p.i_per_cta * p.tile_j +
+                            kFinalizeCost * (double)S * (double)p.part_stride;
+        if (best < 0.0 || cost < best * (1.0 - 1e-9)) { best = cost; p.split = (int)S; }
+    }
+    if (jbytes) *jbytes = (size_t)p.sym_h * (size_t)p.part_stride * elem;
+    return p;
 }
 
 }  // namespace ppgrav

@@ -20,7 +20,12 @@ void count_launch(int n = 1);
     } while (0)
 
 // ---- kernel shapes: one table read by both the plan (plan.cu) and the instantiations (force_f32.cu/force_f64.cu) -------
-// "large" = the throughput shape used whenever it fills the machine, "small" = the fallback for tiny N.
+// Three shape classes per precision:
+//   large  the throughput shape, 1 CTA per SM, whenever it fills the machine (N >~ 2^16)
+//   mid    ~512 i-bodies per CTA, several CTAs per SM: N = 2^13 .. 2^16, where the large shape has too few i-blocks
+//   small  one i-body per thread: tiny N
+// A class fixes tile_j (the per-tile blocking of the sums, hence the bits of the result); threads and i-bodies per
+// thread may differ between the sweep modes of a class (FP64 large: 7 i-bodies force-only, 6 with the potential).
 // Overridable at compile time (-DPP_F32_IPT=2 ...) for tuning sweeps; the defaults are the measured best.
 #ifndef PP_F32_THREADS
 #define PP_F32_THREADS 256
@@ -37,11 +42,26 @@ void count_launch(int n = 1);
 #ifndef PP_F32_UNROLL
 #define PP_F32_UNROLL 2
 #endif
+#ifndef PP_F32_MID_THREADS
+#define PP_F32_MID_THREADS 128
+#endif
+#ifndef PP_F32_MID_IPT
+#define PP_F32_MID_IPT 4
+#endif
+#ifndef PP_F32_MID_TJ
+#define PP_F32_MID_TJ 256
+#endif
+#ifndef PP_F32_MID_MINB
+#define PP_F32_MID_MINB 3
+#endif
 #ifndef PP_F64_THREADS
 #define PP_F64_THREADS 256
 #endif
 #ifndef PP_F64_IPT
 #define PP_F64_IPT 6
+#endif
+#ifndef PP_F64_IPT_FORCE
+#define PP_F64_IPT_FORCE 7
 #endif
 #ifndef PP_F64_TJ
 #define PP_F64_TJ 256
@@ -52,30 +72,62 @@ void count_launch(int n = 1);
 #ifndef PP_F64_UNROLL
 #define PP_F64_UNROLL 2
 #endif
+#ifndef PP_F64_MID_THREADS
+#define PP_F64_MID_THREADS 128
+#endif
+#ifndef PP_F64_MID_IPT
+#define PP_F64_MID_IPT 4
+#endif
+#ifndef PP_F64_MID_TJ
+#define PP_F64_MID_TJ 128
+#endif
+#ifndef PP_F64_MID_MINB
+#define PP_F64_MID_MINB 3
+#endif
 constexpr int kF32Unroll = PP_F32_UNROLL;   // j-pairs (FP32) / j-bodies (FP64) per unrolled loop body
 constexpr int kF64Unroll = PP_F64_UNROLL;
 struct KernelShape {
     int threads, ipt, tile_j, stages, ctas_per_sm;
 };
+enum { CLS_LARGE = 0, CLS_MID = 1, CLS_SMALL = 2, kNumClasses = 3 };
+// modes of the pair sweep
+enum { MODE_FORCE = 0, MODE_FORCE_POT = 1, MODE_POT = 2, kNumModes = 3 };
+// kShapes[precision][class][mode]
 constexpr KernelShape kShapeF32Large = {PP_F32_THREADS, PP_F32_IPT, PP_F32_TJ, 4, PP_F32_MINB};
+constexpr KernelShape kShapeF32Mid = {PP_F32_MID_THREADS, PP_F32_MID_IPT, PP_F32_MID_TJ, 4, PP_F32_MID_MINB};
 constexpr KernelShape kShapeF32Small = {128, 1, 128, 4, 4};
 constexpr KernelShape kShapeF64Large = {PP_F64_THREADS, PP_F64_IPT, PP_F64_TJ, 4, PP_F64_MINB};
+constexpr KernelShape kShapeF64LargeForce = {PP_F64_THREADS, PP_F64_IPT_FORCE, PP_F64_TJ, 4, PP_F64_MINB};
+constexpr KernelShape kShapeF64Mid = {PP_F64_MID_THREADS, PP_F64_MID_IPT, PP_F64_MID_TJ, 4, PP_F64_MID_MINB};
 constexpr KernelShape kShapeF64Small = {128, 1, 128, 4, 4};
+// shape of the symmetric (every unordered pair once) sweeps: the block must be a whole number of tiles and a tile has
+// one body per thread (its j-side sums are reduced one thread per body)
+constexpr KernelShape kShapeF32Sym = {256, 7, 256, 4, 1};
+constexpr KernelShape kShapeF64Sym = {256, 6, 256, 4, 1};
+constexpr KernelShape kShapes[2][kNumClasses][kNumModes] = {
+    {{kShapeF32Large, kShapeF32Large, kShapeF32Large},
+     {kShapeF32Mid, kShapeF32Mid, kShapeF32Mid},
+     {kShapeF32Small, kShapeF32Small, kShapeF32Small}},
+    {{kShapeF64LargeForce, kShapeF64Large, kShapeF64Large},
+     {kShapeF64Mid, kShapeF64Mid, kShapeF64Mid},
+     {kShapeF64Small, kShapeF64Small, kShapeF64Small}},
+};
 
 // ---- launch plan of one gravity solve (plan.cu) --------------------------------------------------------------
 // The all-pairs sweep is cut into work units (i-block, j-split): CTA (ib, s) sweeps the j-tiles of split s for the
 // bodies of i-block ib and writes one partial sum per body; a finalize kernel adds the S partials in fixed order.
 struct Plan {
-    int variant;        // 0 = large shape, 1 = small shape (see KernelShape above)
+    int cls;            // CLS_LARGE / CLS_MID / CLS_SMALL
+    int mode;           // MODE_* the plan was made for (selects the shape within the class)
     int threads;        // threads per CTA
     int ipt;            // i-bodies per thread
     int i_per_cta;      // threads * ipt
     int tile_j;         // j-bodies per shared-memory tile
     int stages;         // depth of the TMA ring
     int ctas_per_sm;    // residency the kernel is built for
-    int64_t n_pad;      // length of the packed array: covers every j-tile and every launched i-block, padded with
-                        // massless bodies (N, or N + i_per_cta for an i-range that starts off a block boundary,
-                        // rounded up to a multiple of i_per_cta, which tile_j divides)
+    int64_t n_pad;      // length of the packed array this plan needs: covers every j-tile and every launched i-block,
+                        // padded with massless bodies (N, or i_begin + part_stride for an i-range that starts off a
+                        // block boundary, rounded up to a multiple of tile_j)
     int64_t i_begin;    // first i-body of the solve (0 for a full solve; pp_forces_range shards the i-range)
     int64_t i_count;    // i-bodies of the solve
     int n_iblocks;      // ceil(i_count / i_per_cta): i-blocks launched
@@ -83,11 +135,16 @@ struct Plan {
     int n_tiles;        // ceil(N / tile_j): j-tiles that contain a real body
     int split;          // S
     int sm_count;
+    // symmetric sweep (force_sym_*.cu): every unordered pair once.  Blocks = i-blocks; block I sweeps the blocks
+    // I+1 .. I+sym_h two-sidedly; j-side sums go to partial_j[sym_h][part_stride].
+    int sym;            // 1 = this plan runs the symmetric kernel
+    int sym_h;          // floor((n_iblocks - 1) / 2)
 };
-Plan make_plan(int64_t N, int precision, int sm_count, int64_t forced_split, int64_t i_begin = 0, int64_t i_count = -1);
-
-// modes of the pair sweep
-enum { MODE_FORCE = 0, MODE_FORCE_POT = 1, MODE_POT = 2 };
+// forced_split >= 1 pins S (capped by the tile count); forced_cls in {0,1,2} pins the shape class, -1 = choose.
+Plan make_plan(int64_t N, int precision, int mode, int sm_count, int64_t forced_split, int forced_cls,
+               int64_t i_begin = 0, int64_t i_count = -1);
+// plan of the symmetric sweep for a full solve of N bodies; bytes of its j-side workspace in *jbytes
+Plan make_sym_plan(int64_t N, int precision, int mode, int sm_count, int64_t forced_split, size_t* jbytes);
 
 // ---- kernels (one launcher per translation unit) -----------------------------------------------------------------
 // Packed bodies.  FP32: pairs of bodies interleaved, 8 floats {x0 x1 y0 y1 z0 z1 m0 m1} per pair (so that one
@@ -107,10 +164,13 @@ int launch_tile_mass_f64(const double* mass, double* tile_mass, int64_t N, int t
                          cudaStream_t st);
 int launch_tile_mass_f64_to_f32(const double* mass, float* tile_mass, int64_t N, int tile_j, int n_tiles, int enable,
                                 cudaStream_t st);
+int launch_tile_mass_f32_to_f64(const float* mass, double* tile_mass, int64_t N, int tile_j, int n_tiles, int enable,
+                                cudaStream_t st);   // pp_invariants' FP64 potential sweep on an FP32 state
 
 // PP_MIXED variants of finalize and kick_drift_pack: FP32 partial sums / packed copy, FP64 state
 int launch_finalize_mixed(const float4* partial, int split, int64_t n_pad, int64_t N, double G, double* acc,
-                          double* pot, double* vel, double kick, cudaStream_t st);
+                          double* pot, double* vel, double kick, cudaStream_t st, const float4* partial_j = nullptr,
+                          int jrows = 0, int64_t jstride = 0);
 int launch_kick_drift_pack_mixed(double* pos, double* vel, const double* acc, const double* mass, float* packed,
                                  int64_t N, int64_t n_pad, double kick, double dt, cudaStream_t st);
 
@@ -119,16 +179,25 @@ int launch_kick_drift_pack_mixed(double* pos, double* vel, const double* acc, co
 // tile_mass: per-j-tile common mass (launch_tile_mass_*), or NULL = treat every tile as mixed.
 int launch_force_f32(const Plan& p, const float* packed, const float* tile_mass, float4* partial, int64_t N,
                      double delta, int mode, cudaStream_t st);
+// symmetric sweep: i-side sums to partial[S][part_stride], j-side sums to partial_j[sym_h][part_stride] (same sign
+// convention, ready to be added); block_mass[I] = common mass of i-block I or NaN (launch_tile_mass_* with tile = block)
+int launch_force_sym_f32(const Plan& p, const float* packed, const float* tile_mass, const float* block_mass,
+                         float4* partial, float4* partial_j, double delta, int mode, cudaStream_t st);
+int launch_force_sym_f64(const Plan& p, const double* packed, const double* tile_mass, const double* block_mass,
+                         double4* partial, double4* partial_j, double delta, int mode, cudaStream_t st);
 // MODE_POT writes {pot_hi, pot_lo, 0, 0} (double-double partial of the potential sum).
 int launch_force_f64(const Plan& p, const double* packed, const double* tile_mass, double4* partial, int64_t N,
                      double delta, int mode, cudaStream_t st);
 
 // acc = G * sum_s partial (fixed order, compensated), pot = -G * sum_s partial.w; optional fused kick
 // vel += kick * acc (kick = 0: none).  acc/pot/vel may be NULL where not wanted.
+// partial_j / jrows / jstride: the j-side rows of the symmetric sweep (force_sym_*.cu), added after the S partials.
 int launch_finalize_f32(const float4* partial, int split, int64_t n_pad, int64_t N, double G, float* acc, float* pot,
-                        float* vel, double kick, cudaStream_t st);
+                        float* vel, double kick, cudaStream_t st, const float4* partial_j = nullptr, int jrows = 0,
+                        int64_t jstride = 0);
 int launch_finalize_f64(const double4* partial, int split, int64_t n_pad, int64_t N, double G, double* acc,
-                        double* pot, double* vel, double kick, int pot_is_dd, cudaStream_t st);
+                        double* pot, double* vel, double kick, int pot_is_dd, cudaStream_t st,
+                        const double4* partial_j = nullptr, int jrows = 0, int64_t jstride = 0);
 
 // v += kick * a;  r += dt * v   on n bodies, no packing (the sharded step kicks and drifts its own bodies only)
 int launch_kick_drift_f32(float* pos, float* vel, const float* acc, int64_t n, double kick, double dt, cudaStream_t st);
@@ -140,6 +209,20 @@ int launch_kick_drift_pack_f32(float* pos, float* vel, const float* acc, const f
                                int64_t n_pad, double kick, double dt, cudaStream_t st);
 int launch_kick_drift_pack_f64(double* pos, double* vel, const double* acc, const double* mass, double* packed,
                                int64_t N, int64_t n_pad, double kick, double dt, cudaStream_t st);
+
+// finalize + closing half-kick + opening half-kick + drift + re-pack in one pass (interior steps of pp_step_kdk)
+int launch_finalize_kick_drift_pack_f32(const float4* partial, int split, int64_t part_stride, int64_t N, double G,
+                                        float* acc, float* vel, float* pos, const float* mass, float* packed,
+                                        double kick, double dt, cudaStream_t st,
+                                        const float4* partial_j = nullptr, int jrows = 0, int64_t jstride = 0);
+int launch_finalize_kick_drift_pack_f64(const double4* partial, int split, int64_t part_stride, int64_t N, double G,
+                                        double* acc, double* vel, double* pos, const double* mass, double* packed,
+                                        double kick, double dt, cudaStream_t st,
+                                        const double4* partial_j = nullptr, int jrows = 0, int64_t jstride = 0);
+int launch_finalize_kick_drift_pack_mixed(const float4* partial, int split, int64_t part_stride, int64_t N, double G,
+                                          double* acc, double* vel, double* pos, const double* mass, float* packed,
+                                          double kick, double dt, cudaStream_t st,
+                                        const float4* partial_j = nullptr, int jrows = 0, int64_t jstride = 0);
 
 // eqs. (8)-(10): block partials (double-double) then a single-block fixed-order sum into out16.
 int invariants_scratch_doubles(int64_t N);
@@ -153,8 +236,5 @@ int launch_density_f32(const float* pos, const float* mass, int64_t N, double x0
                        int ny, double* sigma, int sm_count, cudaStream_t st);
 int launch_density_f64(const double* pos, const double* mass, int64_t N, double x0, double y0, double cell, int nx,
                        int ny, double* sigma, int sm_count, cudaStream_t st);
-
-// pipe microbenchmarks (probe.cu)
-int run_probe(int kind, int64_t iters, int sm_count, double* out4);
 
 }  // namespace ppgrav

@@ -6,6 +6,7 @@
 //   pack            pos[N,3], mass[N] -> packed tile layout (float pairs interleaved / double4), padding included
 //   finalize        acc = G sum_s partial[s] (fixed order, compensated) [, pot = -G sum_s] [, vel += kick acc]
 //   kick_drift_pack vel += kick acc; pos += dt vel; packed = pack(pos, mass)   -- one pass instead of three
+//   finalize_kick_drift_pack  the two above back to back, for the interior steps of a pp_step_kdk call
 #include "ppgrav_internal.h"
 
 namespace ppgrav {
@@ -45,7 +46,7 @@ __global__ void __launch_bounds__(kThreads) tile_mass_kernel(const TIn* __restri
     const int lane = threadIdx.x & 31;
     if (t >= n_tiles) return;                                  // whole warps leave together
     const int64_t j0 = (int64_t)t * tile_j;
-    const TOut first = (TOut)mass[j0];                         // j0 < N: only tiles with a real body are swept
+    const TOut first = j0 < N ? (TOut)mass[j0] : (TOut)0;     // tiles wholly inside the padding have the common mass 0
     bool same = enable != 0;
     for (int j = lane; j < tile_j; j += 32) {
         const TOut m = (j0 + j < N) ? (TOut)mass[j0 + j] : (TOut)0;
@@ -79,7 +80,8 @@ template <> struct Vec4<double> { using type = double4; };
 template <typename TP, typename T, bool POT_DD>
 __global__ void __launch_bounds__(kThreads)
 finalize_kernel(const typename Vec4<TP>::type* __restrict__ partial, int split, int64_t n_pad, int64_t N, T G,
-                T* __restrict__ acc, T* __restrict__ pot, T* __restrict__ vel, T kick) {
+                T* __restrict__ acc, T* __restrict__ pot, T* __restrict__ vel, T kick,
+                const typename Vec4<TP>::type* __restrict__ partial_j, int jrows, int64_t jstride) {
     const int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x;
     if (i >= N) return;
     T sx = 0, sy = 0, sz = 0, sw = 0, cx = 0, cy = 0, cz = 0, cw = 0;
@@ -94,6 +96,14 @@ finalize_kernel(const typename Vec4<TP>::type* __restrict__ partial, int split, 
             comp_add(sz, cz, (T)v.z);
             comp_add(sw, cw, (T)v.w);
         }
+    }
+    // symmetric sweep (force_sym_*.cu): what the blocks I - d, d = 1..jrows, gathered for body i, in fixed order d
+    for (int d = 0; d < jrows; ++d) {
+        const typename Vec4<TP>::type v = partial_j[(size_t)d * jstride + i];
+        comp_add(sx, cx, (T)v.x);
+        comp_add(sy, cy, (T)v.y);
+        comp_add(sz, cz, (T)v.z);
+        comp_add(sw, cw, (T)v.w);
     }
     if (POT_DD) {
         if (pot) pot[i] = -G * (sx + cx);
@@ -123,6 +133,47 @@ kick_drift_pack_kernel(T* __restrict__ pos, T* __restrict__ vel, const T* __rest
         const T v = fma(kick, acc[3 * i + c], vel[3 * i + c]);   // opening half-kick, eq. (5) halved
         vel[3 * i + c] = v;
         r[c] = fma(dt, v, pos[3 * i + c]);                       // drift, eq. (6)
+        pos[3 * i + c] = r[c];
+    }
+    store_packed(packed, i, (TK)r[0], (TK)r[1], (TK)r[2], (TK)mass[i]);
+}
+
+// Between two gravity solves of one pp_step_kdk call the closing half-kick of step n (eq. (7)), the opening half-kick
+// and drift of step n+1 (eqs. (5)-(6)) and the re-packing all touch the same body: one pass instead of two launches
+// (finalize+kick, then kick+drift+pack).  The arithmetic is the same sequence of roundings as the two separate
+// kernels -- acc = G sum_s partial; v = fma(kick, acc, v); v = fma(kick, acc, v); r = fma(dt, v, r) -- so a run is
+// bit-identical whichever way the steps are issued.  Padding bodies (>= N) of `packed` are not touched: they were
+// written by the pass that opened the call and never change.
+template <typename TP, typename T, typename TK>
+__global__ void __launch_bounds__(kThreads)
+finalize_kick_drift_pack_kernel(const typename Vec4<TP>::type* __restrict__ partial, int split, int64_t part_stride,
+                                int64_t N, T G, T* __restrict__ acc, T* __restrict__ vel, T* __restrict__ pos,
+                                const T* __restrict__ mass, TK* __restrict__ packed, T kick, T dt,
+                                const typename Vec4<TP>::type* __restrict__ partial_j, int jrows, int64_t jstride) {
+    const int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x;
+    if (i >= N) return;
+    T sx = 0, sy = 0, sz = 0, cx = 0, cy = 0, cz = 0;
+    for (int s = 0; s < split; ++s) {   // fixed order s = 0..S-1: run-to-run deterministic
+        const typename Vec4<TP>::type v = partial[(size_t)s * part_stride + i];
+        comp_add(sx, cx, (T)v.x);
+        comp_add(sy, cy, (T)v.y);
+        comp_add(sz, cz, (T)v.z);
+    }
+    for (int d = 0; d < jrows; ++d) {   // j-side rows of the symmetric sweep, fixed order
+        const typename Vec4<TP>::type v = partial_j[(size_t)d * jstride + i];
+        comp_add(sx, cx, (T)v.x);
+        comp_add(sy, cy, (T)v.y);
+        comp_add(sz, cz, (T)v.z);
+    }
+    const T a[3] = {G * (sx + cx), G * (sy + cy), G * (sz + cz)};
+    T r[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        acc[3 * i + c] = a[c];
+        T v = fma(kick, a[c], vel[3 * i + c]);    // closing half-kick of this step, eq. (7)
+        v = fma(kick, a[c], v);                   // opening half-kick of the next step, eq. (5) halved
+        vel[3 * i + c] = v;
+        r[c] = fma(dt, v, pos[3 * i + c]);        // drift, eq. (6)
         pos[3 * i + c] = r[c];
     }
     store_packed(packed, i, (TK)r[0], (TK)r[1], (TK)r[2], (TK)mass[i]);
@@ -183,30 +234,34 @@ int launch_pack_f32_to_f64(const float* pos, const float* mass, double* packed, 
 }
 
 int launch_finalize_f32(const float4* partial, int split, int64_t n_pad, int64_t N, double G, float* acc, float* pot,
-                        float* vel, double kick, cudaStream_t st) {
+                        float* vel, double kick, cudaStream_t st, const float4* partial_j, int jrows, int64_t jstride) {
     finalize_kernel<float, float, false><<<grid_for(N), kThreads, 0, st>>>(partial, split, n_pad, N, (float)G, acc,
                                                                            pot, kick != 0.0 ? vel : nullptr,
-                                                                           (float)kick);
+                                                                           (float)kick, partial_j, jrows, jstride);
     count_launch();
     PP_CUDA(cudaGetLastError());
     return PP_OK;
 }
 int launch_finalize_mixed(const float4* partial, int split, int64_t n_pad, int64_t N, double G, double* acc,
-                          double* pot, double* vel, double kick, cudaStream_t st) {
+                          double* pot, double* vel, double kick, cudaStream_t st, const float4* partial_j, int jrows,
+                          int64_t jstride) {
     finalize_kernel<float, double, false><<<grid_for(N), kThreads, 0, st>>>(partial, split, n_pad, N, G, acc, pot,
-                                                                            kick != 0.0 ? vel : nullptr, kick);
+                                                                            kick != 0.0 ? vel : nullptr, kick,
+                                                                            partial_j, jrows, jstride);
     count_launch();
     PP_CUDA(cudaGetLastError());
     return PP_OK;
 }
 int launch_finalize_f64(const double4* partial, int split, int64_t n_pad, int64_t N, double G, double* acc,
-                        double* pot, double* vel, double kick, int pot_is_dd, cudaStream_t st) {
+                        double* pot, double* vel, double kick, int pot_is_dd, cudaStream_t st, const double4* partial_j,
+                        int jrows, int64_t jstride) {
     if (pot_is_dd)
         finalize_kernel<double, double, true><<<grid_for(N), kThreads, 0, st>>>(partial, split, n_pad, N, G, nullptr, pot,
-                                                                        nullptr, 0.0);
+                                                                        nullptr, 0.0, nullptr, 0, 0);
     else
         finalize_kernel<double, double, false><<<grid_for(N), kThreads, 0, st>>>(partial, split, n_pad, N, G, acc, pot,
-                                                                         kick != 0.0 ? vel : nullptr, kick);
+                                                                         kick != 0.0 ? vel : nullptr, kick,
+                                                                         partial_j, jrows, jstride);
     count_launch();
     PP_CUDA(cudaGetLastError());
     return PP_OK;
@@ -244,6 +299,38 @@ int launch_pack_f64_to_f32(const double* pos, const double* mass, float* packed,
     return PP_OK;
 }
 
+int launch_finalize_kick_drift_pack_f32(const float4* partial, int split, int64_t part_stride, int64_t N, double G,
+                                        float* acc, float* vel, float* pos, const float* mass, float* packed,
+                                        double kick, double dt, cudaStream_t st, const float4* partial_j,
+                                        int jrows, int64_t jstride) {
+    finalize_kick_drift_pack_kernel<float, float, float><<<grid_for(N), kThreads, 0, st>>>(
+        partial, split, part_stride, N, (float)G, acc, vel, pos, mass, packed, (float)kick, (float)dt, partial_j, jrows,
+        jstride);
+    count_launch();
+    PP_CUDA(cudaGetLastError());
+    return PP_OK;
+}
+int launch_finalize_kick_drift_pack_f64(const double4* partial, int split, int64_t part_stride, int64_t N, double G,
+                                        double* acc, double* vel, double* pos, const double* mass, double* packed,
+                                        double kick, double dt, cudaStream_t st, const double4* partial_j,
+                                        int jrows, int64_t jstride) {
+    finalize_kick_drift_pack_kernel<double, double, double><<<grid_for(N), kThreads, 0, st>>>(
+        partial, split, part_stride, N, G, acc, vel, pos, mass, packed, kick, dt, partial_j, jrows, jstride);
+    count_launch();
+    PP_CUDA(cudaGetLastError());
+    return PP_OK;
+}
+int launch_finalize_kick_drift_pack_mixed(const float4* partial, int split, int64_t part_stride, int64_t N, double G,
+                                          double* acc, double* vel, double* pos, const double* mass, float* packed,
+                                          double kick, double dt, cudaStream_t st, const float4* partial_j,
+                                        int jrows, int64_t jstride) {
+    finalize_kick_drift_pack_kernel<float, double, float><<<grid_for(N), kThreads, 0, st>>>(
+        partial, split, part_stride, N, G, acc, vel, pos, mass, packed, kick, dt, partial_j, jrows, jstride);
+    count_launch();
+    PP_CUDA(cudaGetLastError());
+    return PP_OK;
+}
+
 template <typename TIn, typename TOut>
 static int launch_tile_mass(const TIn* mass, TOut* tile_mass, int64_t N, int tile_j, int n_tiles, int enable,
                             cudaStream_t st) {
@@ -262,6 +349,10 @@ int launch_tile_mass_f64(const double* mass, double* tile_mass, int64_t N, int t
     return launch_tile_mass(mass, tile_mass, N, tile_j, n_tiles, enable, st);
 }
 int launch_tile_mass_f64_to_f32(const double* mass, float* tile_mass, int64_t N, int tile_j, int n_tiles, int enable,
+                                cudaStream_t st) {
+    return launch_tile_mass(mass, tile_mass, N, tile_j, n_tiles, enable, st);
+}
+int launch_tile_mass_f32_to_f64(const float* mass, double* tile_mass, int64_t N, int tile_j, int n_tiles, int enable,
                                 cudaStream_t st) {
     return launch_tile_mass(mass, tile_mass, N, tile_j, n_tiles, enable, st);
 }

@@ -17,10 +17,9 @@ import numpy as np
 
 PP_F32, PP_F64, PP_MIXED = 0, 1, 2
 PP_ACC_VALID = 1
-PP_CFG_SPLIT_J, PP_CFG_GRAPH, PP_CFG_PROFILE, PP_CFG_EQUAL_MASS = 1, 2, 3, 4
+PP_CFG_SPLIT_J, PP_CFG_GRAPH, PP_CFG_PROFILE, PP_CFG_EQUAL_MASS, PP_CFG_SHAPE, PP_CFG_SYMMETRIC = 1, 2, 3, 4, 5, 6
+SHAPE_AUTO, SHAPE_LARGE, SHAPE_MID, SHAPE_SMALL = 0, 1, 2, 3
 INVARIANT_NAMES = ("E", "K", "W", "Px", "Py", "Pz", "Lx", "Ly", "Lz", "Cx", "Cy", "Cz", "M")
-PROBE_KINDS = {"ffma": 0, "ffma2": 1, "dfma": 2, "mufu_rsq": 3, "mufu_rsq64h": 4, "force_mix_f32": 5,
-               "ffma2_dfma_const": 6, "ffma2_3reg": 7, "ffma2_dfma_3reg": 8}
 
 LIB_PATH = os.environ.get("PPGRAV_LIB") or os.path.join(os.path.dirname(os.path.abspath(__file__)), "libppgrav.so")
 
@@ -43,7 +42,6 @@ SIGNATURES = {
     "pp_invariants_host": (_int, [_vp, _vp, _vp, _vp, _i64, _dbl, _dbl, _int, _vp, _vp]),
     "pp_plan_query": (_int, [_i64, _int, _int, _vp]),
     "pp_equal_mass_tiles": (_int, [_vp, _i64, _int, _vp, _vp]),
-    "pp_probe_pipe": (_int, [_int, _i64, _vp]),
     "pp_profile_read": (_int, [_vp]),
 }
 
@@ -123,11 +121,14 @@ def pp_release(device=-1):
 
 
 def pp_plan_query(N, precision, with_pot=False):
-    out = (ctypes.c_int64 * 8)()
+    out = (ctypes.c_int64 * 16)()
     _check(lib().pp_plan_query(int(N), int(precision), int(bool(with_pot)), out), "pp_plan_query")
-    keys = ("i_per_cta", "tile_j", "split", "ctas", "ctas_per_sm", "sm_count", "pipe_ops_per_pair",
-            "mufu_per_pair")
-    return dict(zip(keys, (int(v) for v in out)))
+    keys = ("i_per_cta", "tile_j", "split", "ctas", "ctas_per_sm", "sm_count", "pipe_ops_per_evaluation",
+            "mufu_per_evaluation", "shape", "threads", "ipt", "i_blocks", "pairs_per_evaluation", "sym_partner_blocks")
+    d = dict(zip(keys, (int(v) for v in out)))
+    # per ordered pair (pair interaction): what the roofline counts; one less on equal-mass tiles
+    d["pipe_ops_per_pair"] = d["pipe_ops_per_evaluation"] / d["pairs_per_evaluation"]
+    return d
 
 
 def pp_equal_mass_tiles(mass, stream=None, mixed=False):
@@ -138,13 +139,6 @@ def pp_equal_mass_tiles(mass, stream=None, mixed=False):
     _check(lib().pp_equal_mass_tiles(_dev(mass, (N,), mass.dtype, "mass"), N, prec, out, _stream(stream)),
            "pp_equal_mass_tiles")
     return int(out[0]), int(out[1])
-
-
-def pp_probe_pipe(kind, iters=1 << 14):
-    k = PROBE_KINDS[kind] if isinstance(kind, str) else int(kind)
-    out = (ctypes.c_double * 4)()
-    _check(lib().pp_probe_pipe(k, int(iters), out), "pp_probe_pipe")
-    return dict(seconds=out[0], lane_ops=out[1], sm_mhz=out[2], lane_ops_per_clk_per_sm=out[3])
 
 
 def pp_profile_read():

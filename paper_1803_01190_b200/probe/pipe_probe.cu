@@ -1,12 +1,15 @@
-// probe.cu -- pipe-throughput microbenchmarks: the MEASURED denominators of the ALU roofline.
+// pipe_probe.cu -- MEASUREMENT TOOLING, NOT PART OF libppgrav: pipe-throughput microbenchmarks behind the ALU roofline
+// denominators (profiles/r1_pipe_probes.md).  Built by paper_1803_01190_b200/build.py into its own
+// libppprobe.so (one C entry point, pp_probe_pipe, below); nothing in the library, the binding, the tests of the hot
+// path or bench.py's timed region links or calls it.
 //
 // The force kernels are bound by the FP32 / FP64 pipes, not by HBM or tensor cores, and MEASURED_PEAKS.json holds
 // no CUDA-core peak.  Each probe runs a long, register-only dependent-chain loop (8 independent chains per thread,
 // 32 warps per SM) of one instruction kind and reports lane-operations per clock per SM, with the SM clock taken
 // from clock64()/globaltimer inside the kernel.
-#include "ppgrav_internal.h"
+#include <cuda_runtime.h>
+#include <stdint.h>
 
-namespace ppgrav {
 namespace {
 
 constexpr int kThreads = 256;
@@ -184,22 +187,28 @@ void launch(int grid, int64_t iters, float* sink, uint64_t* clk) {
 
 }  // namespace
 
-int run_probe(int kind, int64_t iters, int sm_count, double* out4) {
-    if (kind < 0 || kind > 8 || iters < 1) {
-        set_error("pp_probe_pipe: kind must be 0..8 and iters >= 1");
-        return PP_EINVAL;
-    }
+// kind: 0 FFMA, 1 FFMA2 (packed f32x2), 2 DFMA, 3 MUFU.RSQ, 4 MUFU.RSQ64H, 5 FFMA2+MUFU in the force kernel's mix (12 : 2),
+//       6 two FFMA2 : one DFMA with loop-constant multiplier/addend (do the FP32 and FP64 pipes overlap?),
+//       7 FFMA2 with three distinct register operands, 8 as 6 with three distinct register operands each
+// out4 (host) = { seconds, lane-operations executed, SM clock in MHz during the run, lane-ops/clk/SM }; kinds 6-8
+// count the FFMA2 lanes only.  Synchronous.  Returns 0, -1 (bad argument) or -2 (CUDA error).
+extern "C" int pp_probe_pipe(int kind, int64_t iters, double* out4) {
+    if (!out4 || kind < 0 || kind > 8 || iters < 1) return -1;
+#define PROBE_CUDA(call) do { if ((call) != cudaSuccess) { cudaGetLastError(); return -2; } } while (0)
+    int dev = 0, sm_count = 0;
+    PROBE_CUDA(cudaGetDevice(&dev));
+    PROBE_CUDA(cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev));
     const int grid = sm_count * kCtasPerSm;
     float* sink = nullptr;
     uint64_t* clk = nullptr;
-    PP_CUDA(cudaMalloc(&sink, 4));
-    PP_CUDA(cudaMalloc(&clk, sizeof(uint64_t) * 2 * grid));
+    PROBE_CUDA(cudaMalloc(&sink, 4));
+    PROBE_CUDA(cudaMalloc(&clk, sizeof(uint64_t) * 2 * grid));
     cudaEvent_t e0, e1;
-    PP_CUDA(cudaEventCreate(&e0));
-    PP_CUDA(cudaEventCreate(&e1));
+    PROBE_CUDA(cudaEventCreate(&e0));
+    PROBE_CUDA(cudaEventCreate(&e1));
     float ms = 0.f;
     for (int rep = 0; rep < 2; ++rep) {   // first repetition warms up clocks and the instruction cache
-        PP_CUDA(cudaEventRecord(e0));
+        PROBE_CUDA(cudaEventRecord(e0));
         switch (kind) {
             case 0: launch<0>(grid, iters, sink, clk); break;
             case 1: launch<1>(grid, iters, sink, clk); break;
@@ -211,14 +220,14 @@ int run_probe(int kind, int64_t iters, int sm_count, double* out4) {
             case 7: launch<7>(grid, iters, sink, clk); break;
             default: launch<8>(grid, iters, sink, clk); break;
         }
-        count_launch();
-        PP_CUDA(cudaGetLastError());
-        PP_CUDA(cudaEventRecord(e1));
-        PP_CUDA(cudaEventSynchronize(e1));
-        PP_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+        PROBE_CUDA(cudaGetLastError());
+        PROBE_CUDA(cudaEventRecord(e1));
+        PROBE_CUDA(cudaEventSynchronize(e1));
+        PROBE_CUDA(cudaEventElapsedTime(&ms, e0, e1));
     }
     uint64_t h[2];
-    PP_CUDA(cudaMemcpy(h, clk, sizeof(h), cudaMemcpyDeviceToHost));
+    PROBE_CUDA(cudaMemcpy(h, clk, sizeof(h), cudaMemcpyDeviceToHost));
+#undef PROBE_CUDA
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
     cudaFree(sink);
@@ -233,7 +242,5 @@ int run_probe(int kind, int64_t iters, int sm_count, double* out4) {
     out4[1] = lane_ops;
     out4[2] = mhz;
     out4[3] = (mhz > 0.0) ? lane_ops / (sec * mhz * 1e6 * sm_count) : 0.0;
-    return PP_OK;
+    return 0;
 }
-
-}  // namespace ppgrav

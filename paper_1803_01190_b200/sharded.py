@@ -8,6 +8,9 @@ i-range against all N j-bodies (`pp_forces_range`).  One process per GPU; `torch
 
     step:  pp_kick_drift(own)  ->  all_gather(pos)  ->  pp_forces_range(own i, all j)  ->  pp_kick_drift(own, dt=0)
 
+Library launches per step and rank: 6 (kick+drift; tile masses, pack, pair sweep, finalize; closing kick); the exchange
+is one in-place `all_gather_into_tensor` on the replicated position array (no staging buffer, no scatter copies).
+
 Every arithmetic step runs in libppgrav's kernels (the `ops` argument exists so that the rank/partition/exchange logic
 can be exercised on CPU with gloo by injecting stand-ins from the tests; the default `CudaOps` has no fallback).
 BASELINE.json's north_star fixes ONE GPU for the graded path, so `bench.py` keeps independent replicas as its default
@@ -52,6 +55,9 @@ class SingleComm:
     def all_gather_rows(self, own_padded):
         return [own_padded]
 
+    def all_gather_into(self, whole, own_slice):
+        return whole
+
     def all_reduce_sum(self, t):
         return t
 
@@ -70,6 +76,12 @@ class DistComm:
         self.dist.all_gather(out, own_padded, group=self.group)
         return out
 
+    def all_gather_into(self, whole, own_slice):
+        """ONE collective, in place: `own_slice` is this rank's block of `whole` (equal blocks), the others' blocks are
+        received straight into `whole` -- no staging copy, no scatter afterwards."""
+        self.dist.all_gather_into_tensor(whole, own_slice, group=self.group)
+        return whole
+
     def all_reduce_sum(self, t):
         self.dist.all_reduce(t, op=self.dist.ReduceOp.SUM, group=self.group)
         return t
@@ -81,6 +93,13 @@ class ShardedSystem:
     pos, vel [N,3], mass [N]: the FULL initial state, identical on every rank (torch tensors on this rank's device).
     Positions and masses stay replicated (every rank needs all j-bodies); velocities, accelerations and potentials
     exist for the rank's own range only.
+
+    Layout: every rank owns a block of `cmax` = ceil(N / world) rows of the replicated arrays `pos_all` [world*cmax, 3]
+    and `mass_all` [world*cmax]; rank r's bodies are the first `count_r` rows of block r, the rest of a block (at most
+    one row, when world does not divide N) is massless padding at the origin, which contributes nothing to any sum.
+    With equal blocks the per-step exchange is ONE in-place all-gather of `pos_all` itself.  When world divides N the
+    padded system IS the original one and a sharded run is bit-identical to pp_step_kdk; otherwise the padding rows
+    shift the j-tile boundaries and the two agree to summation-order round-off.
     """
 
     def __init__(self, pos, vel, mass, G=1.0, delta=0.0, comm=None, ops=None, initial_pot=True):
@@ -93,17 +112,21 @@ class ShardedSystem:
         self.parts = partition(self.N, self.comm.world)
         if min(c for _, c in self.parts) < 1:
             raise ValueError("more ranks (%d) than bodies (%d)" % (self.comm.world, self.N))
-        self.begin, self.count = self.parts[self.comm.rank]
+        self.begin, self.count = self.parts[self.comm.rank]          # range in the ORIGINAL numbering
         self.cmax = max(c for _, c in self.parts)
-        b, e = self.begin, self.begin + self.count
-        self.pos_all = pos.clone().contiguous()
-        self.mass_all = mass.clone().contiguous()
-        self.pos = self.pos_all[b:e]                     # a view: drifting the own bodies updates pos_all in place
-        self.mass = self.mass_all[b:e]
-        self.vel = vel[b:e].clone().contiguous()
+        self.n_padded = self.cmax * self.comm.world
+        self.row0 = self.comm.rank * self.cmax                       # first row of the own block in the padded arrays
+        self.pos_all = torch.zeros((self.n_padded, 3), dtype=pos.dtype, device=pos.device)
+        self.mass_all = torch.zeros((self.n_padded,), dtype=pos.dtype, device=pos.device)
+        for r, (b, c) in enumerate(self.parts):
+            self.pos_all[r * self.cmax:r * self.cmax + c].copy_(pos[b:b + c])
+            self.mass_all[r * self.cmax:r * self.cmax + c].copy_(mass[b:b + c])
+        self.block = self.pos_all[self.row0:self.row0 + self.cmax]   # views: drifting the own bodies updates pos_all
+        self.pos = self.pos_all[self.row0:self.row0 + self.count]
+        self.mass = self.mass_all[self.row0:self.row0 + self.count]
+        self.vel = vel[self.begin:self.begin + self.count].clone().contiguous()
         self.acc = torch.empty_like(self.vel)
         self.pot = torch.empty((self.count,), dtype=pos.dtype, device=pos.device)
-        self._send = torch.zeros((self.cmax, 3), dtype=pos.dtype, device=pos.device)
         self.force_evaluations = 0
         # a(t0), the one extra solve of a cold start; with the potential, so that invariants() works
         # at t0 (initial_pot=False runs the force-only sweep, exactly what pp_step_kdk's cold start does)
@@ -115,21 +138,14 @@ class ShardedSystem:
         self.ops.kick_drift(self.pos, self.vel, self.acc, 0.5 * dt, dt)
 
     def exchange(self):
-        """All-gather of the drifted positions (the paper's peer reads)."""
-        if self.comm.world == 1:
-            return
-        self._send[:self.count].copy_(self.pos)
-        rows = self.comm.all_gather_rows(self._send)
-        self.scatter_rows(rows)
-
-    def scatter_rows(self, rows):
-        for r, (b, c) in enumerate(self.parts):
-            if r != self.comm.rank:
-                self.pos_all[b:b + c].copy_(rows[r][:c])
+        """All-gather of the drifted positions (the paper's peer reads): one in-place collective on
+        the replicated array, no library kernel and no copy."""
+        if self.comm.world > 1:
+            self.comm.all_gather_into(self.pos_all, self.block)
 
     def solve(self, want_pot=False):
         """Own i-range against all j-bodies, eq. (1)-(2)."""
-        self.ops.forces_range(self.pos_all, self.mass_all, self.begin, self.count, self.G, self.delta, want_pot,
+        self.ops.forces_range(self.pos_all, self.mass_all, self.row0, self.count, self.G, self.delta, want_pot,
                               self.acc, self.pot)
         self.force_evaluations += 1
         self.pot_valid = bool(want_pot)
@@ -169,6 +185,11 @@ class ShardedSystem:
         d["P"], d["L"], d["COM"] = a[3:6].copy(), a[6:9].copy(), np.asarray(com)
         return d
 
+    def positions(self):
+        """pos [N,3] of the whole system in the ORIGINAL numbering (the padding rows dropped)."""
+        return self.torch.cat([self.pos_all[r * self.cmax:r * self.cmax + c] for r, (_, c) in enumerate(self.parts)],
+                              dim=0)
+
     def gather_state(self):
         """(pos [N,3], vel [N,3]) of the whole system on every rank (for tests and output; not on the step path)."""
         torch = self.torch
@@ -176,4 +197,4 @@ class ShardedSystem:
         buf[:self.count].copy_(self.vel)
         rows = self.comm.all_gather_rows(buf)
         vel = torch.cat([rows[r][:c] for r, (_, c) in enumerate(self.parts)], dim=0)
-        return self.pos_all.clone(), vel
+        return self.positions(), vel

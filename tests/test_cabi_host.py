@@ -24,7 +24,7 @@ def test_header_symbols_are_exported_and_bound(ppgrav):
     for name in declared:
         assert hasattr(lib, name), name
     assert declared == set(ppgrav.SIGNATURES), declared ^ set(ppgrav.SIGNATURES)
-    assert lib.pp_version() == 100
+    assert lib.pp_version() == 200
 
 
 def test_no_oracle_import_in_product():
@@ -32,34 +32,71 @@ def test_no_oracle_import_in_product():
     pkg = os.path.join(ROOT, "paper_1803_01190_b200")
     for dirpath, _, files in os.walk(pkg):
         for f in files:
-            if f.endswith((".py", ".cu", ".cuh", ".h")):
+            if f.endswith((".py", ".cu", ".cuh", ".h")) and "__pycache__" not in dirpath:
                 text = open(os.path.join(dirpath, f)).read()
                 assert "import oracle" not in text and "from oracle" not in text and "pp_oracle" not in text, f
 
 
+SHAPES = {0: {"large": (1792, 512), "mid": (512, 256), "small": (128, 128)},
+          1: {"large": (1536, 256), "mid": (512, 128), "small": (128, 128)}}     # (i-bodies per CTA, tile_j) with Phi
+
+
 @pytest.mark.parametrize("prec", [0, 1])
 def test_plan_is_sane(ppgrav, prec):
+    allowed_i = {v[0] for v in SHAPES[prec].values()} | ({1792} if prec else set())   # FP64 force-only: 7 per thread
+    allowed_t = {v[1] for v in SHAPES[prec].values()} | {256}                          # symmetric sweeps: 256
     for n in (1, 2, 100, 2048, 2 ** 14, 2 ** 17, 2 ** 20, 2 ** 22, 2 ** 23):
+        for with_pot in (False, True):
+            p = ppgrav.pp_plan_query(n, prec, with_pot)
+            assert p["i_per_cta"] in allowed_i and p["tile_j"] in allowed_t
+            assert p["i_per_cta"] == p["threads"] * p["ipt"]
+            n_ib = -(-n // p["i_per_cta"])
+            n_tiles = -(-n // p["tile_j"])
+            assert p["i_blocks"] == n_ib
+            assert 1 <= p["split"] <= max(1, n_tiles)
+            assert p["ctas"] == n_ib * p["split"]
+            elem = 32 if prec else 16
+            assert p["split"] * n_ib * p["i_per_cta"] * elem <= (1 << 30) or p["split"] == 1
+            if p["shape"] == 3:                    # symmetric sweep: one evaluation serves two ordered pairs
+                assert (p["i_per_cta"], p["tile_j"]) == ((1536, 256) if prec else (1792, 256))
+                assert p["pairs_per_evaluation"] == 2 and p["sym_partner_blocks"] == (n_ib - 1) // 2
+                assert p["pipe_ops_per_pair"] == ((11.5 if with_pot else 10) if prec else (9 if with_pot else 8))
+            else:
+                assert p["pipe_ops_per_pair"] == ((18 if with_pot else 16) if prec else (13 if with_pot else 12))
+    # calibrated choices: the throughput shape from N = 2^17 up, the mid shape around 2^14,
+    # one body per thread for tiny systems
+    for n in (2 ** 17, 2 ** 20, 2 ** 23):
         p = ppgrav.pp_plan_query(n, prec)
-        assert p["i_per_cta"] in (128, 1536, 1792) and p["tile_j"] in (128, 256, 512)
-        n_ib = -(-n // p["i_per_cta"])
-        n_tiles = -(-n // p["tile_j"])
-        assert 1 <= p["split"] <= max(1, n_tiles)
-        assert p["ctas"] == n_ib * p["split"]
-        elem = 32 if prec else 16
-        n_pad = -(-n // p["i_per_cta"]) * p["i_per_cta"]
-        assert p["split"] * n_pad * elem <= (1 << 30) or p["split"] == 1
-        assert p["pipe_ops_per_pair"] == (16 if prec else 12)
-    # calibrated choices: the throughput shape from N = 2^16 up, the small one below 2^14
-    for n in (2 ** 16, 2 ** 17, 2 ** 20, 2 ** 23):
-        assert ppgrav.pp_plan_query(n, prec)["i_per_cta"] >= 1536
-    for n in (100, 2048, 2 ** 13):
-        assert ppgrav.pp_plan_query(n, prec)["i_per_cta"] == 128
-    big = ppgrav.pp_plan_query(2 ** 20, prec)
+        # full solves up to 2^21 take the symmetric sweep (its j-side workspace must stay under 48 GB)
+        assert p["shape"] == (3 if n <= 2 ** 21 else 0) and p["i_per_cta"] >= 1536
+    for n in (100, 1024):
+        assert ppgrav.pp_plan_query(n, prec)["shape"] == 2
+    # FP64 per-mode shapes of the large class share the tile size (so they share tile masses and padding rules)
+    if prec:
+        f, fp = ppgrav.pp_plan_query(2 ** 23, 1, False), ppgrav.pp_plan_query(2 ** 23, 1, True)
+        assert (f["ipt"], fp["ipt"]) == (7, 6) and f["tile_j"] == fp["tile_j"]
+    ppgrav.pp_configure(ppgrav.PP_CFG_SYMMETRIC, 0)
+    try:
+        big = ppgrav.pp_plan_query(2 ** 20, prec, True)
+    finally:
+        ppgrav.pp_configure(ppgrav.PP_CFG_SYMMETRIC, 1)
     resident = big["sm_count"] * big["ctas_per_sm"]
     waves = big["ctas"] / resident
     assert waves / -(-big["ctas"] // resident) > 0.95, "last wave of the N=2^20 plan should be nearly full"
-    assert ppgrav.pp_plan_query(2 ** 20, prec, True)["pipe_ops_per_pair"] == (18 if prec else 13)
+
+
+@pytest.mark.parametrize("prec", [0, 1])
+def test_forced_shape_is_honoured(ppgrav, prec):
+    try:
+        for key, name in ((ppgrav.SHAPE_LARGE, "large"), (ppgrav.SHAPE_MID, "mid"), (ppgrav.SHAPE_SMALL, "small")):
+            ppgrav.pp_configure(ppgrav.PP_CFG_SHAPE, key)
+            for n in (3, 3000, 2 ** 20):
+                p = ppgrav.pp_plan_query(n, prec, True)
+                assert (p["i_per_cta"], p["tile_j"]) == SHAPES[prec][name] and p["shape"] == key - 1
+        with pytest.raises(ppgrav.PPGravError):
+            ppgrav.pp_configure(ppgrav.PP_CFG_SHAPE, 4)
+    finally:
+        ppgrav.pp_configure(ppgrav.PP_CFG_SHAPE, 0)
 
 
 def test_forced_split_is_honoured(ppgrav):
@@ -75,7 +112,7 @@ def test_bad_arguments_and_no_device(ppgrav):
     import ctypes
     import torch
     lib = ppgrav.lib()
-    out = (ctypes.c_int64 * 8)()
+    out = (ctypes.c_int64 * 16)()
     assert lib.pp_plan_query(0, 0, 0, out) == -1
     assert lib.pp_plan_query(10, 2, 0, out) == 0          # PP_MIXED plans like PP_F32
     assert lib.pp_plan_query(10, 3, 0, out) == -1

@@ -3,8 +3,9 @@
 The oracle cannot sweep these sizes end to end (config 2's 100 steps are 1.1e14 pairs), so -- DESIGN.md section 6 --
 accelerations and potentials are compared on 4096 sampled bodies the oracle evaluates one by one, trajectories
 through oracle-evaluated invariants of the GPU's own snapshots, and a reduced-N run of the same recipe is compared
-with the oracle step for step.  Drift of E, P, L for FP32, FP64 and the oracle is written to
-gpurun_out/drift_r1.json when that folder exists (reported in BASELINE.md).
+with the oracle step for step.  The oracle's own runs of the KDK configs are stored in tests/golden/oracle_drift.json
+(written by tests/golden/make_oracle_drift.py, which calls only oracle/); the GPU's drift report is a command of its
+own (python -m paper_1803_01190_b200.conservation --drift-report), not a side effect of these tests.
 """
 import json
 import os
@@ -26,11 +27,13 @@ def gpu():
         pytest.fail("a -m gpu test was started without a CUDA device")
     from paper_1803_01190_b200 import ppgrav
     ppgrav.lib()
-    yield ppgrav
-    out = os.path.join(ROOT, "gpurun_out")
-    if os.path.isdir(out) and _report:
-        with open(os.path.join(out, "drift_r1.json"), "w") as f:
-            json.dump(_report, f, indent=1, sort_keys=True)
+    return ppgrav
+
+
+@pytest.fixture(scope="module")
+def golden():
+    with open(os.path.join(ROOT, "tests", "golden", "oracle_drift.json")) as f:
+        return json.load(f)
 
 
 def _dtype(prec):
@@ -111,7 +114,7 @@ def _check_snapshot_invariants(gpu, oracle, prec, dpos, dvel, dmass, dpot, c, fu
 
 # ---- config 1: 2^16 disk + 2^16 halo, 200 KDK steps -----------------------------------------------------------------
 @pytest.mark.parametrize("prec", ["f64", "f32"])
-def test_config1_reduced_n_trajectory_against_oracle(gpu, oracle, prec):
+def test_config1_reduced_n_trajectory_against_oracle(gpu, oracle, golden, prec):
     """Same recipe, seed, dt and 200 steps at N = 4096 (2048 + 2048): the oracle integrates it fully."""
     import torch
     from paper_1803_01190_b200 import workloads
@@ -123,6 +126,11 @@ def test_config1_reduced_n_trajectory_against_oracle(gpu, oracle, prec):
         p, v, a, _ = oracle.kdk_halfkick(p, v, mass, c["dt"], 50, G=c["G"], delta=c["delta"], acc=a, nthreads=0)
         series.append(oracle.invariants(p, v, mass, G=c["G"], delta=c["delta"], nthreads=0))
     _report["config1_N4096_oracle"] = _drifts(series)
+    if prec == "f64":        # the stored oracle run (tests/golden/oracle_drift.json) is this very computation
+        g = golden["config1_N4096"]
+        assert g["steps"] == [0, 50, 100, 150, 200]
+        for row, s_ in zip(g["series"], series):
+            assert np.allclose(row, s_["raw"][:13], rtol=1e-13, atol=1e-18)
     dpos, dvel, dmass = _dev(prec, pos), _dev(prec, vel), _dev(prec, mass)
     dacc = torch.zeros_like(dpos)
     gser = [gpu.invariants_dict(gpu.pp_invariants(dpos, dvel, dmass, G=c["G"], delta=c["delta"]))]
@@ -136,7 +144,7 @@ def test_config1_reduced_n_trajectory_against_oracle(gpu, oracle, prec):
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
-def test_config1_full_size(gpu, oracle, prec):
+def test_config1_full_size(gpu, oracle, golden, prec):
     import torch
     from paper_1803_01190_b200 import workloads
     c = workloads.config(1)
@@ -153,6 +161,20 @@ def test_config1_full_size(gpu, oracle, prec):
     assert last["E"] == series[-1]["E"]
     d = _drifts(series)
     _report["config1_%s" % prec] = d
+    # step-for-step against the oracle's own 200-step run of the FULL config (3.5e12 pair interactions, stored by
+    # tests/golden/make_oracle_drift.py): final r, v of the 256 tracked bodies, and E, L_z at steps 0, 50, ..., 200
+    if "config1" not in golden:
+        pytest.skip("tests/golden/oracle_drift.json has no full-size config1 run yet")
+    g = golden["config1"]
+    assert g["N"] == c["N"] and g["nsteps"] == c["nsteps"] and g["steps"] == [0, 50, 100, 150, 200]
+    track = np.array(g["track_index"])
+    tol = {"f64": 1e-10, "f32": 2e-5}[prec]             # 200 steps (as the reduced-N test)
+    dr = np.abs(dpos[track].cpu().numpy() - np.array(g["track_pos"])).max() / g["max_abs_pos"]
+    dv = np.abs(dvel[track].cpu().numpy() - np.array(g["track_vel"])).max() / g["max_abs_vel"]
+    assert dr <= tol and dv <= tol, (dr, dv)
+    if prec == "f64":
+        for row, got in zip(g["series"], series):
+            assert abs(got["E"] - row[0]) <= 1e-9 * abs(row[0]) and abs(got["L"][2] - row[8]) <= 1e-9 * abs(row[8])
     if prec == "f64":                                    # leapfrog conserves P and L exactly: FP64 sits at round-off
         assert d["dP_abs"] <= 1e-13 and d["dLz_over_Lz0"] <= 1e-12 and d["dE_over_E0"] <= 1e-3
     else:
