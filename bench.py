@@ -377,16 +377,18 @@ def run_sweep_n(args):
             pot = torch.empty_like(mass)
             peak = lanes * SM_COUNT * SM_MAX_HZ
             for shape, key, symkey in shapes:
-                if shape == "small" and logn > 17 or shape == "mid" and logn > 20 or shape == "symmetric" and logn > 21:
+                if (shape == "small" and logn > 17 or shape == "mid" and logn > 20 or
+                        logn > 21 and shape not in ("auto", "large")):
                     continue                           # far outside their range: minutes per solve, nothing to learn
+                                                       # (above 2^21: the library's own choice and the large one-sided class)
                 ppgrav.pp_configure(ppgrav.PP_CFG_SHAPE, key)
                 ppgrav.pp_configure(ppgrav.PP_CFG_SYMMETRIC, symkey)
-                for with_pot in (False, True):
+                for with_pot in ((False,) if logn > 21 else (False, True)):
                     plan = ppgrav.pp_plan_query(N, code, with_pot)
                     est = pairs * (12 if name == "f32" else 17) / (0.5 * peak)          # rough seconds per solve
                     if shape == "small":
                         est *= 2.5
-                    reps = int(max(2, min(20, 1.0 / max(est, 1e-4))))
+                    reps = int(max(1 if logn > 21 else 2, min(20, 1.0 / max(est, 1e-4))))
                     times = []
                     for r in range(reps + 1):
                         flush_buf.zero_()

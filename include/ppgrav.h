@@ -74,9 +74,15 @@ extern "C" {
 
 #define PP_CFG_SYMMETRIC 6 /* the pair sweep that evaluates every UNORDERED pair once (Newton's third law: one evaluation
                             * of eq. (2) serves i <- j and j <- i; 7-9 instead of 11-13 FP32-pipe operations per pair
-                            * interaction).  1 (default) = used for full solves with an FP32 sweep (PP_F32, PP_MIXED)
-                            * when the plan would take the large shape class and its j-side workspace
-                            * (N^2/3584 x 16 B) stays under 32 GB, i.e. 2^16 < N <= 2^21; 0 = never; 2 = always */
+                            * interaction, 9-11.5 instead of 15-18 FP64).  1 (default) = used for full solves (every
+                            * precision; not for i-ranges) of N >= 49152 bodies, if its j-side workspace (N^2/(2B) x 16
+                            * or 32 B, B = 2048, at most 48 GB; in bands of 16 GB beyond N = 2^21) can be
+                            * allocated -- otherwise the one-sided sweep runs; 0 = never; 2 = always (PP_ENOMEM if the
+                            * workspace cannot be allocated) */
+
+#define PP_CFG_SYM_BAND_ROWS 7 /* test hook: 0 (default) = the symmetric sweep keeps all its j-side rows when they fit 48 GB
+                                * and otherwise works through bands of partner offsets of at most 16 GB of rows;
+                                * r >= 1 = bands of at most r partner offsets */
 
 /* Version of the library that was loaded (PPGRAV_VERSION). */
 int pp_version(void);
@@ -174,7 +180,8 @@ int pp_invariants_host(const void* pos, const void* vel, const void* mass, const
  *     [7] MUFU operations per evaluation, [8] shape class (0 large, 1 mid, 2 small, 3 = the symmetric sweep,
  *     PP_CFG_SYMMETRIC), [9] threads per CTA, [10] i-bodies per thread, [11] i-blocks,
  *     [12] ordered pairs (pair interactions) one evaluation serves: 1, or 2 for the symmetric sweep,
- *     [13] symmetric sweep: partner blocks H per block (rows of its j-side workspace), [14], [15] reserved }. */
+ *     [13] symmetric sweep: partner blocks H per block, [14] symmetric sweep: bands the partner blocks are cut into
+ *     (1 = all j-side rows are kept at once), [15] reserved }. */
 int pp_plan_query(int64_t N, int precision, int with_pot, int64_t* out16);
 
 /* How many j-tiles of a gravity solve of these masses have a common mass (and therefore run the pair loop without

@@ -28,15 +28,18 @@ std::atomic<int64_t> g_cfg_profile{0};
 std::atomic<int64_t> g_cfg_equal_mass{1};
 std::atomic<int64_t> g_cfg_shape{0};
 std::atomic<int64_t> g_cfg_symmetric{1};
+std::atomic<int64_t> g_cfg_band_rows{0};
 std::vector<std::pair<cudaEvent_t, cudaEvent_t>> g_prof;   // guarded by g_mu (every sweep is launched under it)
 
 constexpr int kMaxDevices = 64;
 constexpr int64_t kMaxN = (int64_t)1 << 28;
-constexpr int kNumBuf = 7;
-enum { B_PACKED = 0, B_PARTIAL, B_INV, B_POT64, B_TILE_MASS, B_PARTIAL_J, B_BLOCK_MASS };
-// the j-side rows of the symmetric sweep grow as N^2 / (2 x 1792) x 16 B: 4.9 GB at N = 2^20, 19.6 GB at 2^21; above
-// this cap a solve falls back to the one-sided sweep
+constexpr int kNumBuf = 8;
+enum { B_PACKED = 0, B_PARTIAL, B_INV, B_POT64, B_TILE_MASS, B_PARTIAL_J, B_BLOCK_MASS, B_ACC_J };
+// the j-side rows of the symmetric sweep grow as N^2 / (2 x 2048) x 16 B (FP64: 32 B): 4.3 GB at N = 2^20, 17 GB at 2^21.  Up to
+// kMaxPartialJBytes they are kept whole (one sweep launch, finalize reads them directly); beyond, the partner offsets
+// are cut into bands of at most kBandBytes whose rows are reused and folded into running sums
 constexpr size_t kMaxPartialJBytes = (size_t)48 << 30;
+constexpr size_t kBandBytes = (size_t)16 << 30;
 
 // one instantiated CUDA graph of an interior KDK step (sweep + finalize_kick_drift_pack), reused while every
 // kernel argument it was recorded with is unchanged
@@ -149,7 +152,8 @@ size_t sweep_elem_bytes(int precision) { return precision == PP_F64 ? 8 : 4; }
 
 // the pair sweep, optionally bracketed by events (PP_CFG_PROFILE)
 int sweep(const Plan& p, int precision, const void* packed, const void* tile_mass, void* partial, int64_t N,
-          double delta, int mode, cudaStream_t st, const void* block_mass = nullptr, void* partial_j = nullptr) {
+          double delta, int mode, cudaStream_t st, const void* block_mass = nullptr, void* partial_j = nullptr,
+          void* acc_j = nullptr) {
     const bool prof = g_cfg_profile.load() != 0;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (prof) {
@@ -160,10 +164,10 @@ int sweep(const Plan& p, int precision, const void* packed, const void* tile_mas
     int rc;
     if (p.sym && sweep_precision(precision) == PP_F32)
         rc = launch_force_sym_f32(p, (const float*)packed, (const float*)tile_mass, (const float*)block_mass,
-                                  (float4*)partial, (float4*)partial_j, delta, mode, st);
+                                  (float4*)partial, (float4*)partial_j, (float4*)acc_j, delta, mode, st);
     else if (p.sym)
         rc = launch_force_sym_f64(p, (const double*)packed, (const double*)tile_mass, (const double*)block_mass,
-                                  (double4*)partial, (double4*)partial_j, delta, mode, st);
+                                  (double4*)partial, (double4*)partial_j, (double4*)acc_j, delta, mode, st);
     else
         rc = sweep_precision(precision) == PP_F32
                  ? launch_force_f32(p, (const float*)packed, (const float*)tile_mass, (float4*)partial, N, delta, mode, st)
@@ -176,24 +180,35 @@ int sweep(const Plan& p, int precision, const void* packed, const void* tile_mas
     return rc;
 }
 
+// where finalize finds the j-side sums of a symmetric sweep, and how many i-side partials there are per body
+struct JSide {
+    const void* ptr;
+    int rows, split;
+};
+JSide jside(const Plan& p, const void* partial_j, const void* acc_j) {
+    if (!p.sym) return {nullptr, 0, p.split};
+    if (p.sym_bands > 1) return {acc_j, 2, p.split * p.sym_bands};   // running TwoSum (value, error) of the bands
+    return {partial_j, p.sym_h, p.split};
+}
+
 // one gravity solve on already packed bodies: sweep + finalize (optionally with the closing half-kick)
 // (acc, pot, vel address the p.i_count bodies of the plan's i-range; p must be the plan of the mode pot selects;
 // block_mass / partial_j: the symmetric sweep's extra input and j-side rows, unused otherwise)
 int solve_packed(const Plan& p, int precision, const void* packed, const void* tile_mass, void* partial, int64_t N,
                  double G, double delta, void* acc, void* pot, void* vel, double kick, cudaStream_t st,
-                 const void* block_mass = nullptr, void* partial_j = nullptr) {
+                 const void* block_mass = nullptr, void* partial_j = nullptr, void* acc_j = nullptr) {
     const int mode = pot ? MODE_FORCE_POT : MODE_FORCE;
-    PP_TRY(sweep(p, precision, packed, tile_mass, partial, N, delta, mode, st, block_mass, partial_j));
-    const int jrows = p.sym ? p.sym_h : 0;
+    PP_TRY(sweep(p, precision, packed, tile_mass, partial, N, delta, mode, st, block_mass, partial_j, acc_j));
+    const JSide j = jside(p, partial_j, acc_j);
     if (precision == PP_F32)
-        return launch_finalize_f32((const float4*)partial, p.split, p.part_stride, p.i_count, G, (float*)acc,
-                                   (float*)pot, (float*)vel, kick, st, (const float4*)partial_j, jrows, p.part_stride);
+        return launch_finalize_f32((const float4*)partial, j.split, p.part_stride, p.i_count, G, (float*)acc,
+                                   (float*)pot, (float*)vel, kick, st, (const float4*)j.ptr, j.rows, p.part_stride);
     if (precision == PP_MIXED)
-        return launch_finalize_mixed((const float4*)partial, p.split, p.part_stride, p.i_count, G, (double*)acc,
-                                     (double*)pot, (double*)vel, kick, st, (const float4*)partial_j, jrows,
+        return launch_finalize_mixed((const float4*)partial, j.split, p.part_stride, p.i_count, G, (double*)acc,
+                                     (double*)pot, (double*)vel, kick, st, (const float4*)j.ptr, j.rows,
                                      p.part_stride);
-    return launch_finalize_f64((const double4*)partial, p.split, p.part_stride, p.i_count, G, (double*)acc,
-                               (double*)pot, (double*)vel, kick, 0, st, (const double4*)partial_j, jrows,
+    return launch_finalize_f64((const double4*)partial, j.split, p.part_stride, p.i_count, G, (double*)acc,
+                               (double*)pot, (double*)vel, kick, 0, st, (const double4*)j.ptr, j.rows,
                                p.part_stride);
 }
 
@@ -255,7 +270,7 @@ struct Solve {
     Plan force, force_pot;
     int64_t n_pad = 0;
     void *packed = nullptr, *partial = nullptr, *tm = nullptr;
-    void *partial_j = nullptr, *bm = nullptr;   // symmetric sweep only
+    void *partial_j = nullptr, *bm = nullptr, *acc_j = nullptr;   // symmetric sweep only
     const Plan& plan(int mode) const { return mode == MODE_FORCE ? force : force_pot; }
 };
 
@@ -269,11 +284,17 @@ bool symmetric_plan(int64_t N, int sweep_prec, int mode, int sm_count, bool full
     if (cfg == 0 || !full || (mode != MODE_FORCE && mode != MODE_FORCE_POT)) return false;
     if (cfg == 1) {   // automatic: not when a shape class is pinned (PP_CFG_SHAPE addresses the one-sided kernels)
         if (forced_class() >= 0) return false;
-        if (make_plan(N, sweep_prec, mode, sm_count, 0, -1).cls != CLS_LARGE) return false;
+        // measured: faster than the large one-sided class from N = 2^16 on, slower at 2^15
+        if (N < 49152 || make_plan(N, sweep_prec, mode, sm_count, 0, -1).cls != CLS_LARGE) return false;
     }
-    size_t jbytes = 0;
-    const Plan sp = make_sym_plan(N, sweep_prec, mode, sm_count, g_cfg_split.load(), &jbytes);
-    if (jbytes > kMaxPartialJBytes) return false;
+    size_t jbytes = 0, abytes = 0;
+    Plan sp = make_sym_plan(N, sweep_prec, mode, sm_count, g_cfg_split.load(), kMaxPartialJBytes, &jbytes, &abytes);
+    if (sp.sym_bands > 1) sp = make_sym_plan(N, sweep_prec, mode, sm_count, g_cfg_split.load(), kBandBytes, &jbytes, &abytes);
+    const int64_t force_rows = g_cfg_band_rows.load();   // PP_CFG_SYM_BAND_ROWS (tests): at most that many rows per band
+    if (force_rows >= 1) {
+        const size_t row_bytes = (size_t)sp.part_stride * (sweep_prec == PP_F64 ? 32 : 16);
+        sp = make_sym_plan(N, sweep_prec, mode, sm_count, g_cfg_split.load(), (size_t)force_rows * row_bytes, &jbytes, &abytes);
+    }
     *p = sp;
     return true;
 }
@@ -286,7 +307,17 @@ int prepare_solve(Workspace* w, int64_t N, int precision, const void* mass, bool
     // the class is chosen for the mode that dominates the call
     const int lead = want_force_only ? MODE_FORCE : MODE_FORCE_POT;
     Plan first;
-    const bool sym = symmetric_plan(N, sp, lead, w->sm_count, full, &first);
+    bool sym = symmetric_plan(N, sp, lead, w->sm_count, full, &first);
+    if (sym) {   // its j-side rows are the one big allocation of the library: if HBM cannot hold them, sweep one-sidedly
+        const size_t row_bytes = (size_t)first.part_stride * 4 * sweep_elem_bytes(precision);
+        const size_t jb = std::max<size_t>((size_t)std::min(first.sym_rows, std::max(first.sym_h, 1)) * row_bytes, 16);
+        if (ensure(w, B_PARTIAL_J, jb, &s->partial_j) != PP_OK ||
+            (first.sym_bands > 1 && ensure(w, B_ACC_J, 2 * row_bytes, &s->acc_j) != PP_OK)) {
+            if (g_cfg_symmetric.load() == 2) return PP_ENOMEM;   // pinned by the caller: report, do not fall back
+            set_error("");
+            sym = false;
+        }
+    }
     if (sym) {
         s->force = s->force_pot = first;
         s->force.mode = MODE_FORCE;
@@ -300,14 +331,13 @@ int prepare_solve(Workspace* w, int64_t N, int precision, const void* mass, bool
     }
     s->n_pad = std::max(s->force.n_pad, s->force_pot.n_pad);
     const size_t body = 4 * sweep_elem_bytes(precision);
-    const size_t part = std::max((size_t)s->force.split * (size_t)s->force.part_stride,
-                                 (size_t)s->force_pot.split * (size_t)s->force_pot.part_stride);
+    const size_t bands = sym ? (size_t)first.sym_bands : 1;   // a banded symmetric sweep keeps S partials per band
+    const size_t part = bands * std::max((size_t)s->force.split * (size_t)s->force.part_stride,
+                                         (size_t)s->force_pot.split * (size_t)s->force_pot.part_stride);
     PP_TRY(ensure(w, B_PACKED, (size_t)s->n_pad * body, &s->packed));
     PP_TRY(ensure(w, B_PARTIAL, part * body, &s->partial));
     if (mass) PP_TRY(tile_masses(w, first, precision, mass, N, (int)g_cfg_equal_mass.load(), &s->tm, st));
     if (sym) {
-        PP_TRY(ensure(w, B_PARTIAL_J, std::max<size_t>((size_t)first.sym_h * (size_t)first.part_stride * body, 16),
-                      &s->partial_j));
         PP_TRY(ensure(w, B_BLOCK_MASS, (size_t)first.n_iblocks * sweep_elem_bytes(precision), &s->bm));
         if (mass) {   // common mass per i-block: the same kernel with tile = block
             const int em = (int)g_cfg_equal_mass.load();
@@ -327,20 +357,20 @@ int prepare_solve(Workspace* w, int64_t N, int precision, const void* mass, bool
 // finalize + closing kick + opening kick + drift + re-pack (interior steps of pp_step_kdk)
 int finalize_kick_drift_pack(const Plan& p, int precision, const void* partial, int64_t N, double G, void* acc,
                              void* vel, void* pos, const void* mass, void* packed, double kick, double dt,
-                             cudaStream_t st, const void* partial_j = nullptr) {
-    const int jrows = p.sym ? p.sym_h : 0;
+                             cudaStream_t st, const void* partial_j = nullptr, const void* acc_j = nullptr) {
+    const JSide j = jside(p, partial_j, acc_j);
     if (precision == PP_F32)
-        return launch_finalize_kick_drift_pack_f32((const float4*)partial, p.split, p.part_stride, N, G, (float*)acc,
+        return launch_finalize_kick_drift_pack_f32((const float4*)partial, j.split, p.part_stride, N, G, (float*)acc,
                                                    (float*)vel, (float*)pos, (const float*)mass, (float*)packed, kick,
-                                                   dt, st, (const float4*)partial_j, jrows, p.part_stride);
+                                                   dt, st, (const float4*)j.ptr, j.rows, p.part_stride);
     if (precision == PP_MIXED)
-        return launch_finalize_kick_drift_pack_mixed((const float4*)partial, p.split, p.part_stride, N, G,
+        return launch_finalize_kick_drift_pack_mixed((const float4*)partial, j.split, p.part_stride, N, G,
                                                      (double*)acc, (double*)vel, (double*)pos, (const double*)mass,
-                                                     (float*)packed, kick, dt, st, (const float4*)partial_j, jrows,
+                                                     (float*)packed, kick, dt, st, (const float4*)j.ptr, j.rows,
                                                      p.part_stride);
-    return launch_finalize_kick_drift_pack_f64((const double4*)partial, p.split, p.part_stride, N, G, (double*)acc,
+    return launch_finalize_kick_drift_pack_f64((const double4*)partial, j.split, p.part_stride, N, G, (double*)acc,
                                                (double*)vel, (double*)pos, (const double*)mass, (double*)packed, kick,
-                                               dt, st, (const double4*)partial_j, jrows, p.part_stride);
+                                               dt, st, (const double4*)j.ptr, j.rows, p.part_stride);
 }
 
 }  // namespace
@@ -379,6 +409,7 @@ int pp_configure(int key, int64_t value) {
     if (key == PP_CFG_EQUAL_MASS && (value == 0 || value == 1)) { g_cfg_equal_mass.store(value); return PP_OK; }
     if (key == PP_CFG_SHAPE && value >= 0 && value <= kNumClasses) { g_cfg_shape.store(value); return PP_OK; }
     if (key == PP_CFG_SYMMETRIC && value >= 0 && value <= 2) { g_cfg_symmetric.store(value); return PP_OK; }
+    if (key == PP_CFG_SYM_BAND_ROWS && value >= 0 && value <= (1 << 20)) { g_cfg_band_rows.store(value); return PP_OK; }
     set_error("pp_configure: unknown key %d or value %lld out of range", key, (long long)value);
     return PP_EINVAL;
 }
@@ -473,7 +504,8 @@ int pp_plan_query(int64_t N, int precision, int with_pot, int64_t* out16) {
     out12[11] = p.n_iblocks;
     out16[12] = p.sym ? 2 : 1;
     out16[13] = p.sym ? p.sym_h : 0;
-    out16[14] = out16[15] = 0;
+    out16[14] = p.sym ? p.sym_bands : 0;
+    out16[15] = 0;
     return PP_OK;
 }
 
@@ -527,7 +559,7 @@ int pp_forces_range(const void* pos, const void* mass, void* acc, void* pot, int
     PP_TRY(prepare_solve(w, N, precision, mass, pot == nullptr, st, &s, i_begin, i_count));
     PP_TRY(pack_state(precision, pos, mass, s.packed, N, s.n_pad, st));
     PP_TRY(solve_packed(s.plan(pot ? MODE_FORCE_POT : MODE_FORCE), precision, s.packed, s.tm, s.partial, N, G, delta,
-                        acc, pot, nullptr, 0.0, st, s.bm, s.partial_j));
+                        acc, pot, nullptr, 0.0, st, s.bm, s.partial_j, s.acc_j));
     return leave(w, st);
 }
 
@@ -581,7 +613,7 @@ int pp_step_kdk(void* pos, void* vel, const void* mass, void* acc, void* pot, in
         void* pot0 = nsteps == 0 ? pot : nullptr;
         PP_TRY(pack_state(precision, pos, mass, s.packed, N, s.n_pad, st));
         PP_TRY(solve_packed(s.plan(pot0 ? MODE_FORCE_POT : MODE_FORCE), precision, s.packed, s.tm, s.partial, N, G,
-                            delta, acc, pot0, nullptr, 0.0, st, s.bm, s.partial_j));
+                            delta, acc, pot0, nullptr, 0.0, st, s.bm, s.partial_j, s.acc_j));
     }
     if (nsteps == 0) return leave(w, st);
     const double half = 0.5 * dt;
@@ -600,7 +632,7 @@ int pp_step_kdk(void* pos, void* vel, const void* mass, void* acc, void* pot, in
     key.pos = pos; key.vel = vel; key.mass = mass; key.acc = acc; key.packed = s.packed; key.partial = s.partial;
     key.tm = s.tm; key.N = N; key.n_pad = s.n_pad; key.part_stride = pf.part_stride; key.precision = precision;
     key.cls = pf.cls; key.split = pf.split; key.threads = pf.threads; key.ipt = pf.ipt; key.dt = dt; key.G = G;
-    key.delta = delta; key.sym = pf.sym; key.partial_j = s.partial_j;
+    key.delta = delta; key.sym = pf.sym * 1000 + pf.sym_bands; key.partial_j = s.partial_j;
     const StepGraph& g = w->graph;
     const bool hit = g.exec && g.pos == key.pos && g.vel == key.vel && g.mass == key.mass && g.acc == key.acc &&
                      g.packed == key.packed && g.partial == key.partial && g.tm == key.tm && g.N == key.N &&
@@ -626,10 +658,10 @@ int pp_step_kdk(void* pos, void* vel, const void* mass, void* acc, void* pot, in
             drop_graph(w);
             cudaGraph_t graph = nullptr;
             PP_CUDA(cudaStreamBeginCapture(run, cudaStreamCaptureModeThreadLocal));
-            int rc = sweep(pf, precision, s.packed, s.tm, s.partial, N, delta, MODE_FORCE, run, s.bm, s.partial_j);
+            int rc = sweep(pf, precision, s.packed, s.tm, s.partial, N, delta, MODE_FORCE, run, s.bm, s.partial_j, s.acc_j);
             if (rc == PP_OK)
                 rc = finalize_kick_drift_pack(pf, precision, s.partial, N, G, acc, vel, pos, mass, s.packed, half, dt,
-                                              run, s.partial_j);
+                                              run, s.partial_j, s.acc_j);
             const cudaError_t ec = cudaStreamEndCapture(run, &graph);
             count_launch(-2);   // the two captured launches were recorded, not run
             if (rc != PP_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
@@ -652,13 +684,13 @@ int pp_step_kdk(void* pos, void* vel, const void* mass, void* acc, void* pot, in
         }
     } else {
         for (int64_t k = 0; k < nbody; ++k) {
-            PP_TRY(sweep(pf, precision, s.packed, s.tm, s.partial, N, delta, MODE_FORCE, st, s.bm, s.partial_j));
+            PP_TRY(sweep(pf, precision, s.packed, s.tm, s.partial, N, delta, MODE_FORCE, st, s.bm, s.partial_j, s.acc_j));
             PP_TRY(finalize_kick_drift_pack(pf, precision, s.partial, N, G, acc, vel, pos, mass, s.packed, half, dt, st,
-                                            s.partial_j));
+                                            s.partial_j, s.acc_j));
         }
     }
     PP_TRY(solve_packed(s.plan(pot ? MODE_FORCE_POT : MODE_FORCE), precision, s.packed, s.tm, s.partial, N, G, delta,
-                        acc, pot, vel, half, st, s.bm, s.partial_j));
+                        acc, pot, vel, half, st, s.bm, s.partial_j, s.acc_j));
     return leave(w, st);
 }
 

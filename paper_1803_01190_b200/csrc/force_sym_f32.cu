@@ -3,9 +3,11 @@
 // eq. (2) is antisymmetric: m_i f_ij = -m_j f_ji.  The ordered-pair sweep of force_f32.cu spends 11 FP32-pipe
 // operations on every (i <- j) and again on (j <- i); here one evaluation of r_j - r_i, r^2 + delta^2 and its -3/2 power
 // feeds BOTH bodies: 14 packed operations per two ordered pairs (7 per ordered pair; 8 with the potential or with
-// unequal masses) instead of 11 (12).  The pipe is as busy as before -- the work per pair interaction shrinks.
+// unequal masses) instead of 11 (12).  The work per pair interaction shrinks by a third; the pipe runs at ~0.76 instead
+// of ~0.86 of its peak, because six of the fourteen instructions now read three distinct 64-bit register operands
+// (ncu: math-pipe throttle and fixed-latency waits, profiles/r2_force_sym_f32_ncu.md).
 //
-//  * Bodies are cut into blocks of B = THREADS x IPT (1792).  Block I owns the unordered block pairs (I, I+d),
+//  * Bodies are cut into blocks of B = THREADS x IPT (256 x 8 = 2048).  Block I owns the unordered block pairs (I, I+d),
 //    d = 1 .. H = floor((nb-1)/2), cyclically: every pair of distinct blocks exactly once, the same load for every I.
 //    Its own block (and, for an even number of blocks, the block opposite, I + nb/2, which two CTAs share) is swept the
 //    ordinary one-sided way (sweep_tile of force_f32_common.cuh): B/N of the work.
@@ -14,13 +16,17 @@
 //    i-bodies on it; 32 systolic steps rotate the j-pairs (and their accumulators) through the lanes by warp shuffles,
 //    so after 32 steps each of the 64 j-bodies has met all 32 x IPT i-bodies of the warp.  No shared-memory traffic in
 //    the pair loop at all; 12-16 shuffles per 14 pair evaluations.
-//  * i-side sums stay in registers exactly as in force_f32.cu (per-tile packed sums folded into TwoSum outer sums).
+//  * i-side per-tile packed sums stay in registers exactly as in force_f32.cu; the TwoSum outer sums they are folded
+//    into once per tile live in shared memory, which frees the registers for 8 i-bodies per thread (measured: 7 % faster
+//    than 7, the shuffles being shared by more pair work).
 //    j-side sums of the 8 warps meet in shared memory once per tile and go to partial_j[d-1][j]; update.cu's finalize
 //    adds, for every body, its S i-side partials and its H j-side partials in fixed order.  No atomics anywhere:
 //    bit-reproducible run to run.
 //  * Equal-mass shortcut as in force_f32.cu, now needing a common mass on both sides (the j-tile's, applied to the i-side
 //    fold; the i-block's, applied to the j-side reduction).  Otherwise m_j w^3 and m_i w^3 are formed per pair.
 #include "force_f32_common.cuh"
+#include <algorithm>
+
 #include "tma_ring.cuh"
 
 namespace ppgrav {
@@ -30,53 +36,59 @@ __device__ __forceinline__ float2 rot(const float2 v, const int src) {
     return make_float2(__shfl_sync(0xffffffffu, v.x, src), __shfl_sync(0xffffffffu, v.y, src));
 }
 
-// One chunk of a tile: 64 j-bodies (this lane starts with the j-pair (xj, yj, zj, mj)) against the warp's 32 x IPT
-// i-bodies.  On return (fx, fy, fz, fp) holds, for the j-pair this lane STARTED with, sum_i [m_i] w^3 (r_j - r_i) and
-// sum_i [m_i] w over the warp's i-bodies ([m_i] only when !UNI), and the i-side packed sums have grown accordingly.
-template <int IPT, int MODE, bool GUARD, bool UNI>
-__device__ __forceinline__ void sym_chunk(float2 xj, float2 yj, float2 zj, float2 mj, const float2 (&nx)[IPT],
-                                          const float2 (&ny)[IPT], const float2 (&nz)[IPT], const float2 (&mi)[IPT],
-                                          float2 (&ax)[IPT], float2 (&ay)[IPT], float2 (&az)[IPT], float2 (&ap)[IPT],
-                                          float2& fx, float2& fy, float2& fz, float2& fp, const float2 eps2,
-                                          const int lane) {
-    fx = fy = fz = fp = make_float2(0.f, 0.f);
+// One chunk of a tile: JP x 64 j-bodies (this lane starts with the j-pairs (xj, yj, zj, mj)[0..JP)) against the warp's
+// 32 x IPT i-bodies.  On return (fx, fy, fz, fp)[q] holds, for the q-th j-pair this lane STARTED with,
+// sum_i [m_i] w^3 (r_j - r_i) and sum_i [m_i] w over the warp's i-bodies ([m_i] only when !UNI), and the i-side packed
+// sums have grown accordingly.  JP > 1 keeps independent j-pairs in flight, so that the shuffles of one overlap the
+// arithmetic of the other.
+template <int IPT, int JP, int MODE, bool GUARD, bool UNI>
+__device__ __forceinline__ void sym_chunk(float2 (&xj)[JP], float2 (&yj)[JP], float2 (&zj)[JP], float2 (&mj)[JP],
+                                          const float2 (&nx)[IPT], const float2 (&ny)[IPT], const float2 (&nz)[IPT],
+                                          const float2 (&mi)[IPT], float2 (&ax)[IPT], float2 (&ay)[IPT],
+                                          float2 (&az)[IPT], float2 (&ap)[IPT], float2 (&fx)[JP], float2 (&fy)[JP],
+                                          float2 (&fz)[JP], float2 (&fp)[JP], const float2 eps2, const int lane) {
+#pragma unroll
+    for (int q = 0; q < JP; ++q) fx[q] = fy[q] = fz[q] = fp[q] = make_float2(0.f, 0.f);
     const int src = (lane + 1) & 31;
-#pragma unroll 2
+#pragma unroll kSymF32Unroll
     for (int step = 0; step < 32; ++step) {
 #pragma unroll
-        for (int k = 0; k < IPT; ++k) {
-            const float2 dx = __fadd2_rn(xj, nx[k]);          // r_j - r_i (two j-bodies)
-            const float2 dy = __fadd2_rn(yj, ny[k]);
-            const float2 dz = __fadd2_rn(zj, nz[k]);
-            float2 r2 = __ffma2_rn(dx, dx, eps2);             // |r_i - r_j|^2 + delta^2
-            r2 = __ffma2_rn(dy, dy, r2);
-            r2 = __ffma2_rn(dz, dz, r2);
-            float2 w;
-            w.x = rsqrt_approx(r2.x);
-            w.y = rsqrt_approx(r2.y);
-            if (GUARD) {
-                w.x = r2.x > kTinyR2F32 ? w.x : 0.f;
-                w.y = r2.y > kTinyR2F32 ? w.y : 0.f;
+        for (int q = 0; q < JP; ++q) {
+#pragma unroll
+            for (int k = 0; k < IPT; ++k) {
+                const float2 dx = __fadd2_rn(xj[q], nx[k]);          // r_j - r_i (two j-bodies)
+                const float2 dy = __fadd2_rn(yj[q], ny[k]);
+                const float2 dz = __fadd2_rn(zj[q], nz[k]);
+                float2 r2 = __ffma2_rn(dx, dx, eps2);                // |r_i - r_j|^2 + delta^2
+                r2 = __ffma2_rn(dy, dy, r2);
+                r2 = __ffma2_rn(dz, dz, r2);
+                float2 w;
+                w.x = rsqrt_approx(r2.x);
+                w.y = rsqrt_approx(r2.y);
+                if (GUARD) {
+                    w.x = r2.x > kTinyR2F32 ? w.x : 0.f;
+                    w.y = r2.y > kTinyR2F32 ? w.y : 0.f;
+                }
+                const float2 w3 = __fmul2_rn(w, __fmul2_rn(w, w));
+                const float2 si = UNI ? w3 : __fmul2_rn(mj[q], w3);  // pull of j on i:  m_j w^3 (r_j - r_i)
+                const float2 sj = UNI ? w3 : __fmul2_rn(mi[k], w3);  // pull of i on j: -m_i w^3 (r_j - r_i), sign in the reduction
+                ax[k] = __ffma2_rn(si, dx, ax[k]);
+                ay[k] = __ffma2_rn(si, dy, ay[k]);
+                az[k] = __ffma2_rn(si, dz, az[k]);
+                fx[q] = __ffma2_rn(sj, dx, fx[q]);
+                fy[q] = __ffma2_rn(sj, dy, fy[q]);
+                fz[q] = __ffma2_rn(sj, dz, fz[q]);
+                if (MODE == MODE_FORCE_POT) {
+                    ap[k] = UNI ? __fadd2_rn(ap[k], w) : __ffma2_rn(mj[q], w, ap[k]);
+                    fp[q] = UNI ? __fadd2_rn(fp[q], w) : __ffma2_rn(mi[k], w, fp[q]);
+                }
             }
-            const float2 w3 = __fmul2_rn(w, __fmul2_rn(w, w));
-            const float2 si = UNI ? w3 : __fmul2_rn(mj, w3);     // pull of j on i:  m_j w^3 (r_j - r_i)
-            const float2 sj = UNI ? w3 : __fmul2_rn(mi[k], w3);  // pull of i on j: -m_i w^3 (r_j - r_i), sign in the reduction
-            ax[k] = __ffma2_rn(si, dx, ax[k]);
-            ay[k] = __ffma2_rn(si, dy, ay[k]);
-            az[k] = __ffma2_rn(si, dz, az[k]);
-            fx = __ffma2_rn(sj, dx, fx);
-            fy = __ffma2_rn(sj, dy, fy);
-            fz = __ffma2_rn(sj, dz, fz);
-            if (MODE == MODE_FORCE_POT) {
-                ap[k] = UNI ? __fadd2_rn(ap[k], w) : __ffma2_rn(mj, w, ap[k]);
-                fp = UNI ? __fadd2_rn(fp, w) : __ffma2_rn(mi[k], w, fp);
-            }
+            // systolic step: this j-pair, with the sums it has gathered, moves one lane down
+            xj[q] = rot(xj[q], src); yj[q] = rot(yj[q], src); zj[q] = rot(zj[q], src);
+            if (!UNI) mj[q] = rot(mj[q], src);
+            fx[q] = rot(fx[q], src); fy[q] = rot(fy[q], src); fz[q] = rot(fz[q], src);
+            if (MODE == MODE_FORCE_POT) fp[q] = rot(fp[q], src);
         }
-        // systolic step: every j-pair, with the sums it has gathered, moves one lane down
-        xj = rot(xj, src); yj = rot(yj, src); zj = rot(zj, src);
-        if (!UNI) mj = rot(mj, src);
-        fx = rot(fx, src); fy = rot(fy, src); fz = rot(fz, src);
-        if (MODE == MODE_FORCE_POT) fp = rot(fp, src);
     }   // after 32 rotations every pair is back in the lane it started in
 }
 
@@ -84,14 +96,15 @@ template <int THREADS, int IPT, int TJ, int STAGES, int MODE, bool GUARD>
 __global__ void __launch_bounds__(THREADS, 1)
 force_sym_f32_kernel(const float* __restrict__ packed, const float* __restrict__ tile_mass,
                      const float* __restrict__ block_mass, float4* __restrict__ partial,
-                     float4* __restrict__ partial_j, const int nb, const int H, const int64_t part_stride,
+                     float4* __restrict__ partial_j, const int nb, const int d0, const int rows, const int first, const int64_t part_stride,
                      const int64_t n_padb, const float eps2f) {
     constexpr int NWARPS = THREADS / 32;
     constexpr int B = THREADS * IPT;
     constexpr int TPB = B / TJ;            // j-tiles per block
-    constexpr int CHUNKS = TJ / 64;        // 64 j-bodies (32 lanes x one pair) per systolic pass
+    constexpr int JP = kSymF32Jp;          // j-pairs a lane keeps in flight
+    constexpr int CHUNKS = TJ / (64 * JP); // JP x 64 j-bodies (32 lanes x JP pairs) per systolic pass
     constexpr uint32_t TILE_BYTES = TJ * 16u;
-    static_assert(B % TJ == 0 && TJ % 64 == 0 && TJ == THREADS, "one thread per j-body in the tile reduction");
+    static_assert(B % TJ == 0 && TJ % (64 * JP) == 0 && TJ == THREADS, "one thread per j-body in the tile reduction");
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float* tiles = reinterpret_cast<float*>(smem_raw);                                   // [STAGES][TJ*4]
     float2* jacc = reinterpret_cast<float2*>(smem_raw + STAGES * TILE_BYTES);            // [2][NWARPS][TJ/2][4]
@@ -102,14 +115,16 @@ force_sym_f32_kernel(const float* __restrict__ packed, const float* __restrict__
     const int I = blockIdx.x;
     const int S = gridDim.y, sidx = blockIdx.y;
     // non-symmetric tiles (split 0 only): the own block, and for an even block count the opposite block I + nb/2
-    const int n_ns = sidx == 0 ? TPB * ((nb > 1 && (nb & 1) == 0) ? 2 : 1) : 0;
-    const int P = H * TPB;                 // symmetric partner tiles of block I: blocks I+1 .. I+H (cyclic)
+    // (a solve whose j-side rows do not fit the workspace at once is cut into bands of partner offsets d0+1 .. d0+rows;
+    // the non-symmetric tiles belong to the first band)
+    const int n_ns = (sidx == 0 && first) ? TPB * ((nb > 1 && (nb & 1) == 0) ? 2 : 1) : 0;
+    const int P = rows * TPB;                 // symmetric partner tiles of block I: blocks I+1 .. I+H (cyclic)
     const int p0 = (int)(((int64_t)P * sidx) / S), p1 = (int)(((int64_t)P * (sidx + 1)) / S);
     const int nt = n_ns + (p1 - p0);
     auto tile_of = [&](int q) -> int {
         if (q < n_ns) return ((q < TPB ? I : (I + nb / 2) % nb)) * TPB + q % TPB;
         const int p = p0 + (q - n_ns);
-        return ((I + 1 + p / TPB) % nb) * TPB + p % TPB;
+        return ((I + 1 + d0 + p / TPB) % nb) * TPB + p % TPB;
     };
 
     if (tid == 0) {
@@ -131,7 +146,10 @@ force_sym_f32_kernel(const float* __restrict__ packed, const float* __restrict__
 
     float2 nx[IPT], ny[IPT], nz[IPT], mi[IPT];
     float2 ax[IPT], ay[IPT], az[IPT], ap[IPT];
-    float sx[IPT], sy[IPT], sz[IPT], sp[IPT], cx[IPT], cy[IPT], cz[IPT], cp[IPT];
+    // compensated outer sums (value, error) x (x, y, z, phi) per i-body: touched once per tile, so they live in shared
+    // memory -- osum[q][k][tid], q = 0..7 -- and leave their 8 IPT registers to more i-bodies per thread
+    float* osum = reinterpret_cast<float*>(empty_bar + STAGES);
+    auto os = [&](int q, int k) -> float& { return osum[(q * IPT + k) * THREADS + tid]; };
     int iidx[IPT];
 #pragma unroll
     for (int k = 0; k < IPT; ++k) {
@@ -144,8 +162,8 @@ force_sym_f32_kernel(const float* __restrict__ packed, const float* __restrict__
         nz[k] = make_float2(-zi, -zi);
         mi[k] = make_float2(m, m);
         ax[k] = ay[k] = az[k] = ap[k] = make_float2(0.f, 0.f);
-        sx[k] = sy[k] = sz[k] = sp[k] = 0.f;
-        cx[k] = cy[k] = cz[k] = cp[k] = 0.f;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) os(q, k) = 0.f;
     }
     const float2 eps2 = make_float2(eps2f, eps2f);
     const float bm = block_mass ? __ldg(block_mass + I) : __int_as_float(0x7fc00000);   // common mass of the own block
@@ -177,20 +195,27 @@ force_sym_f32_kernel(const float* __restrict__ packed, const float* __restrict__
             float2* mine = jacc + ((size_t)(buf * NWARPS + warp) * (TJ / 2)) * 4;
 #pragma unroll 1
             for (int c = 0; c < CHUNKS; ++c) {
-                const float4 a = tp[2 * (c * 32 + lane)];
-                const float4 b = tp[2 * (c * 32 + lane) + 1];
-                float2 fx, fy, fz, fp;
+                float2 xj[JP], yj[JP], zj[JP], mj[JP], fx[JP], fy[JP], fz[JP], fp[JP];
+#pragma unroll
+                for (int q = 0; q < JP; ++q) {
+                    const float4 a = tp[2 * ((c * JP + q) * 32 + lane)];
+                    const float4 b = tp[2 * ((c * JP + q) * 32 + lane) + 1];
+                    xj[q] = make_float2(a.x, a.y); yj[q] = make_float2(a.z, a.w);
+                    zj[q] = make_float2(b.x, b.y); mj[q] = make_float2(b.z, b.w);
+                }
                 if (uni)
-                    sym_chunk<IPT, MODE, GUARD, true>(make_float2(a.x, a.y), make_float2(a.z, a.w), make_float2(b.x, b.y),
-                                                      make_float2(b.z, b.w), nx, ny, nz, mi, ax, ay, az, ap, fx, fy, fz,
-                                                      fp, eps2, lane);
+                    sym_chunk<IPT, JP, MODE, GUARD, true>(xj, yj, zj, mj, nx, ny, nz, mi, ax, ay, az, ap, fx, fy, fz, fp,
+                                                          eps2, lane);
                 else
-                    sym_chunk<IPT, MODE, GUARD, false>(make_float2(a.x, a.y), make_float2(a.z, a.w), make_float2(b.x, b.y),
-                                                       make_float2(b.z, b.w), nx, ny, nz, mi, ax, ay, az, ap, fx, fy, fz,
-                                                       fp, eps2, lane);
-                float4* o = reinterpret_cast<float4*>(mine + (size_t)(c * 32 + lane) * 4);
-                o[0] = make_float4(fx.x, fx.y, fy.x, fy.y);
-                o[1] = make_float4(fz.x, fz.y, (MODE == MODE_FORCE_POT) ? fp.x : 0.f, (MODE == MODE_FORCE_POT) ? fp.y : 0.f);
+                    sym_chunk<IPT, JP, MODE, GUARD, false>(xj, yj, zj, mj, nx, ny, nz, mi, ax, ay, az, ap, fx, fy, fz, fp,
+                                                           eps2, lane);
+#pragma unroll
+                for (int q = 0; q < JP; ++q) {
+                    float4* o = reinterpret_cast<float4*>(mine + (size_t)((c * JP + q) * 32 + lane) * 4);
+                    o[0] = make_float4(fx[q].x, fx[q].y, fy[q].x, fy[q].y);
+                    o[1] = make_float4(fz[q].x, fz[q].y, (MODE == MODE_FORCE_POT) ? fp[q].x : 0.f,
+                                       (MODE == MODE_FORCE_POT) ? fp[q].y : 0.f);
+                }
             }
         }
         const float scale = uni ? tm : 1.0f;
@@ -208,12 +233,16 @@ force_sym_f32_kernel(const float* __restrict__ packed, const float* __restrict__
         // i-side: fold the tile's packed partial sums into the compensated outer sums
 #pragma unroll
         for (int k = 0; k < IPT; ++k) {
-            comp_add(sx[k], cx[k], __fmul_rn(scale, __fadd_rn(ax[k].x, ax[k].y)));
-            comp_add(sy[k], cy[k], __fmul_rn(scale, __fadd_rn(ay[k].x, ay[k].y)));
-            comp_add(sz[k], cz[k], __fmul_rn(scale, __fadd_rn(az[k].x, az[k].y)));
+            float v0 = os(0, k), e0 = os(1, k), v1 = os(2, k), e1 = os(3, k), v2 = os(4, k), e2 = os(5, k);
+            comp_add(v0, e0, __fmul_rn(scale, __fadd_rn(ax[k].x, ax[k].y)));
+            comp_add(v1, e1, __fmul_rn(scale, __fadd_rn(ay[k].x, ay[k].y)));
+            comp_add(v2, e2, __fmul_rn(scale, __fadd_rn(az[k].x, az[k].y)));
+            os(0, k) = v0; os(1, k) = e0; os(2, k) = v1; os(3, k) = e1; os(4, k) = v2; os(5, k) = e2;
             ax[k] = ay[k] = az[k] = make_float2(0.f, 0.f);
             if (MODE == MODE_FORCE_POT) {
-                comp_add(sp[k], cp[k], __fmul_rn(scale, __fadd_rn(ap[k].x, ap[k].y)));
+                float v3 = os(6, k), e3 = os(7, k);
+                comp_add(v3, e3, __fmul_rn(scale, __fadd_rn(ap[k].x, ap[k].y)));
+                os(6, k) = v3; os(7, k) = e3;
                 ap[k] = make_float2(0.f, 0.f);
             }
         }
@@ -243,33 +272,42 @@ force_sym_f32_kernel(const float* __restrict__ packed, const float* __restrict__
 #pragma unroll
     for (int k = 0; k < IPT; ++k) {
         float4 o;
-        o.x = __fadd_rn(sx[k], cx[k]);
-        o.y = __fadd_rn(sy[k], cy[k]);
-        o.z = __fadd_rn(sz[k], cz[k]);
-        o.w = (MODE == MODE_FORCE_POT) ? __fadd_rn(sp[k], cp[k]) : 0.f;
+        o.x = __fadd_rn(os(0, k), os(1, k));
+        o.y = __fadd_rn(os(2, k), os(3, k));
+        o.z = __fadd_rn(os(4, k), os(5, k));
+        o.w = (MODE == MODE_FORCE_POT) ? __fadd_rn(os(6, k), os(7, k)) : 0.f;
         partial[(size_t)sidx * part_stride + iidx[k]] = o;
     }
 }
 
 template <int MODE, bool GUARD>
 int launch_mg(const Plan& p, const float* packed, const float* tile_mass, const float* block_mass, float4* partial,
-              float4* partial_j, float eps2, cudaStream_t st) {
+              float4* partial_j, float4* acc_j, float eps2, cudaStream_t st) {
     constexpr KernelShape K = kShapeF32Sym;
-    constexpr size_t smem = (size_t)K.stages * K.tile_j * 16 + 2 * (K.threads / 32) * (K.tile_j / 2) * 32 + 2 * K.stages * 8;
+    // j-tile ring + two j-side reduction buffers + mbarriers + the outer sums
+    constexpr size_t smem = (size_t)K.stages * K.tile_j * 16 + 2 * (K.threads / 32) * (K.tile_j / 2) * 32 + 2 * K.stages * 8 +
+                            (size_t)8 * K.ipt * K.threads * 4;
     auto kern = force_sym_f32_kernel<K.threads, K.ipt, K.tile_j, K.stages, MODE, GUARD>;
     PP_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));   // > 48 KB: opt-in
     dim3 grid(p.n_iblocks, p.split);
-    kern<<<grid, K.threads, smem, st>>>(packed, tile_mass, block_mass, partial, partial_j, p.n_iblocks, p.sym_h,
-                                        p.part_stride, p.part_stride, eps2);
-    count_launch();
-    PP_CUDA(cudaGetLastError());
+    // bands of partner offsets (one band unless the j-side rows exceed the workspace cap): band b writes its i-side
+    // partials behind those of band b-1 and reuses the j-side rows, which fold_rows (update.cu) adds up in between
+    for (int b = 0; b < p.sym_bands; ++b) {
+        const int d0 = b * p.sym_rows, rows = std::min(p.sym_rows, p.sym_h - d0);
+        kern<<<grid, K.threads, smem, st>>>(packed, tile_mass, block_mass,
+                                            partial + (size_t)b * p.split * p.part_stride, partial_j, p.n_iblocks, d0,
+                                            rows, b == 0, p.part_stride, p.part_stride, eps2);
+        count_launch();
+        PP_CUDA(cudaGetLastError());
+        if (p.sym_bands > 1) PP_TRY_RC(launch_fold_rows(partial_j, rows, p.part_stride, acc_j, b == 0, st));
+    }
     return PP_OK;
 }
 
 }  // namespace
 
 int launch_force_sym_f32(const Plan& p, const float* packed, const float* tile_mass, const float* block_mass,
-                         float4* partial, float4* partial_j, double delta, int mode, cudaStream_t st) {
+                         float4* partial, float4* partial_j, float4* acc_j, double delta, int mode, cudaStream_t st) {
     constexpr KernelShape K = kShapeF32Sym;
     if (!p.sym || p.threads != K.threads || p.ipt != K.ipt || p.tile_j != K.tile_j || p.i_begin != 0) {
         set_error("launch_force_sym_f32: not a symmetric FP32 plan");
@@ -278,10 +316,10 @@ int launch_force_sym_f32(const Plan& p, const float* packed, const float* tile_m
     const float eps2 = (float)(delta * delta);
     const bool guard = !(eps2 >= kTinyR2F32);
     if (mode == MODE_FORCE)
-        return guard ? launch_mg<MODE_FORCE, true>(p, packed, tile_mass, block_mass, partial, partial_j, eps2, st)
-                     : launch_mg<MODE_FORCE, false>(p, packed, tile_mass, block_mass, partial, partial_j, eps2, st);
-    return guard ? launch_mg<MODE_FORCE_POT, true>(p, packed, tile_mass, block_mass, partial, partial_j, eps2, st)
-                 : launch_mg<MODE_FORCE_POT, false>(p, packed, tile_mass, block_mass, partial, partial_j, eps2, st);
+        return guard ? launch_mg<MODE_FORCE, true>(p, packed, tile_mass, block_mass, partial, partial_j, acc_j, eps2, st)
+                     : launch_mg<MODE_FORCE, false>(p, packed, tile_mass, block_mass, partial, partial_j, acc_j, eps2, st);
+    return guard ? launch_mg<MODE_FORCE_POT, true>(p, packed, tile_mass, block_mass, partial, partial_j, acc_j, eps2, st)
+                 : launch_mg<MODE_FORCE_POT, false>(p, packed, tile_mass, block_mass, partial, partial_j, acc_j, eps2, st);
 }
 
 }  // namespace ppgrav

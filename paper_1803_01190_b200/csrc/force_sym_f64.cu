@@ -2,12 +2,14 @@
 //
 // The FP64 twin of force_sym_f32.cu (read its header for the block-pair decomposition, the systolic rotation of the
 // j-bodies through the lanes of a warp, and the fixed-order j-side reduction).  What differs: one j-body per lane (no
-// packed FP64 arithmetic exists), 32 j-bodies per systolic pass, i-blocks of 256 x 6 = 1536 bodies, and the
+// packed FP64 arithmetic exists), 32 j-bodies per systolic pass, and the
 // RSQ64H-seed-plus-one-cubic-correction reciprocal square root of force_f64.cu.  FP64-pipe operations per evaluation,
 // which serves the two ordered pairs (i <- j) and (j <- i): 18 force-only (15 one-sided per ORDERED pair), 21 with the
 // potential (17), two more when the masses are not common to block and tile -- 9 / 10.5 instead of 15 / 17 per pair
 // interaction.
 #include "force_f64_common.cuh"
+#include <algorithm>
+
 #include "tma_ring.cuh"
 
 namespace ppgrav {
@@ -27,7 +29,7 @@ __device__ __forceinline__ void sym_chunk(double xj, double yj, double zj, doubl
                                           const int lane) {
     fx = fy = fz = fp = 0.0;
     const int src = (lane + 1) & 31;
-#pragma unroll 2
+#pragma unroll kSymF64Unroll
     for (int step = 0; step < 32; ++step) {
 #pragma unroll
         for (int k = 0; k < IPT; ++k) {
@@ -73,7 +75,7 @@ template <int THREADS, int IPT, int TJ, int STAGES, int MODE, bool GUARD>
 __global__ void __launch_bounds__(THREADS, 1)
 force_sym_f64_kernel(const double* __restrict__ packed, const double* __restrict__ tile_mass,
                      const double* __restrict__ block_mass, double4* __restrict__ partial,
-                     double4* __restrict__ partial_j, const int nb, const int H, const int64_t part_stride,
+                     double4* __restrict__ partial_j, const int nb, const int d0, const int rows, const int first, const int64_t part_stride,
                      const int64_t n_padb, const double eps2) {
     constexpr int NWARPS = THREADS / 32;
     constexpr int B = THREADS * IPT;
@@ -90,14 +92,16 @@ force_sym_f64_kernel(const double* __restrict__ packed, const double* __restrict
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int I = blockIdx.x;
     const int S = gridDim.y, sidx = blockIdx.y;
-    const int n_ns = sidx == 0 ? TPB * ((nb > 1 && (nb & 1) == 0) ? 2 : 1) : 0;
-    const int P = H * TPB;
+    // (a solve whose j-side rows do not fit the workspace at once is cut into bands of partner offsets d0+1 .. d0+rows;
+    // the non-symmetric tiles belong to the first band)
+    const int n_ns = (sidx == 0 && first) ? TPB * ((nb > 1 && (nb & 1) == 0) ? 2 : 1) : 0;
+    const int P = rows * TPB;
     const int p0 = (int)(((int64_t)P * sidx) / S), p1 = (int)(((int64_t)P * (sidx + 1)) / S);
     const int nt = n_ns + (p1 - p0);
     auto tile_of = [&](int q) -> int {
         if (q < n_ns) return ((q < TPB ? I : (I + nb / 2) % nb)) * TPB + q % TPB;
         const int p = p0 + (q - n_ns);
-        return ((I + 1 + p / TPB) % nb) * TPB + p % TPB;
+        return ((I + 1 + d0 + p / TPB) % nb) * TPB + p % TPB;
     };
 
     if (tid == 0) {
@@ -119,7 +123,9 @@ force_sym_f64_kernel(const double* __restrict__ packed, const double* __restrict
 
     double xi[IPT], yi[IPT], zi[IPT], mi[IPT];
     double ax[IPT], ay[IPT], az[IPT], ap[IPT];
-    double sx[IPT], sy[IPT], sz[IPT], sp[IPT];
+    // outer sums (x, y, z, phi) per i-body: touched once per tile, so they live in shared memory (osum[q][k][tid])
+    double* osum = reinterpret_cast<double*>(empty_bar + STAGES);
+    auto os = [&](int q, int k) -> double& { return osum[(q * IPT + k) * THREADS + tid]; };
     int iidx[IPT];
 #pragma unroll
     for (int k = 0; k < IPT; ++k) {
@@ -128,7 +134,7 @@ force_sym_f64_kernel(const double* __restrict__ packed, const double* __restrict
         const double4 q = reinterpret_cast<const double4*>(packed)[i];
         xi[k] = q.x; yi[k] = q.y; zi[k] = q.z; mi[k] = q.w;
         ax[k] = ay[k] = az[k] = ap[k] = 0.0;
-        sx[k] = sy[k] = sz[k] = sp[k] = 0.0;
+        os(0, k) = os(1, k) = os(2, k) = os(3, k) = 0.0;
     }
     const double kNoCommonMass = __longlong_as_double(0x7ff8000000000000ll);
     const double bm = block_mass ? __ldg(block_mass + I) : kNoCommonMass;
@@ -183,9 +189,11 @@ force_sym_f64_kernel(const double* __restrict__ packed, const double* __restrict
 
 #pragma unroll
         for (int k = 0; k < IPT; ++k) {
-            sx[k] = fma(scale, ax[k], sx[k]); sy[k] = fma(scale, ay[k], sy[k]); sz[k] = fma(scale, az[k], sz[k]);
+            os(0, k) = fma(scale, ax[k], os(0, k));
+            os(1, k) = fma(scale, ay[k], os(1, k));
+            os(2, k) = fma(scale, az[k], os(2, k));
             ax[k] = ay[k] = az[k] = 0.0;
-            if (MODE == MODE_FORCE_POT) { sp[k] = fma(scale, ap[k], sp[k]); ap[k] = 0.0; }
+            if (MODE == MODE_FORCE_POT) { os(3, k) = fma(scale, ap[k], os(3, k)); ap[k] = 0.0; }
         }
 
         if (sym) {   // j-side: the 8 warps' sums for the TJ bodies of this tile, added in warp order, one thread per body
@@ -208,28 +216,38 @@ force_sym_f64_kernel(const double* __restrict__ packed, const double* __restrict
 #pragma unroll
     for (int k = 0; k < IPT; ++k)
         partial[(size_t)sidx * part_stride + iidx[k]] =
-            make_double4(sx[k], sy[k], sz[k], (MODE == MODE_FORCE_POT) ? sp[k] : 0.0);
+            make_double4(os(0, k), os(1, k), os(2, k), (MODE == MODE_FORCE_POT) ? os(3, k) : 0.0);
 }
 
 template <int MODE, bool GUARD>
 int launch_mg(const Plan& p, const double* packed, const double* tile_mass, const double* block_mass, double4* partial,
-              double4* partial_j, double eps2, cudaStream_t st) {
+              double4* partial_j, double4* acc_j, double eps2, cudaStream_t st) {
     constexpr KernelShape K = kShapeF64Sym;
-    constexpr size_t smem = (size_t)K.stages * K.tile_j * 32 + 2 * (K.threads / 32) * K.tile_j * 32 + 2 * K.stages * 8;
+    // j-tile ring + two j-side reduction buffers + mbarriers + the outer sums
+    constexpr size_t smem = (size_t)K.stages * K.tile_j * 32 + 2 * (K.threads / 32) * K.tile_j * 32 + 2 * K.stages * 8 +
+                            (size_t)4 * K.ipt * K.threads * 8;
+    static_assert(smem <= 227 * 1024, "shared memory of the symmetric FP64 sweep");
     auto kern = force_sym_f64_kernel<K.threads, K.ipt, K.tile_j, K.stages, MODE, GUARD>;
     PP_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));   // > 48 KB: opt-in
     dim3 grid(p.n_iblocks, p.split);
-    kern<<<grid, K.threads, smem, st>>>(packed, tile_mass, block_mass, partial, partial_j, p.n_iblocks, p.sym_h,
-                                        p.part_stride, p.part_stride, eps2);
-    count_launch();
-    PP_CUDA(cudaGetLastError());
+    // bands of partner offsets (one band unless the j-side rows exceed the workspace cap): band b writes its i-side
+    // partials behind those of band b-1 and reuses the j-side rows, which fold_rows (update.cu) adds up in between
+    for (int b = 0; b < p.sym_bands; ++b) {
+        const int d0 = b * p.sym_rows, rows = std::min(p.sym_rows, p.sym_h - d0);
+        kern<<<grid, K.threads, smem, st>>>(packed, tile_mass, block_mass,
+                                            partial + (size_t)b * p.split * p.part_stride, partial_j, p.n_iblocks, d0,
+                                            rows, b == 0, p.part_stride, p.part_stride, eps2);
+        count_launch();
+        PP_CUDA(cudaGetLastError());
+        if (p.sym_bands > 1) PP_TRY_RC(launch_fold_rows(partial_j, rows, p.part_stride, acc_j, b == 0, st));
+    }
     return PP_OK;
 }
 
 }  // namespace
 
 int launch_force_sym_f64(const Plan& p, const double* packed, const double* tile_mass, const double* block_mass,
-                         double4* partial, double4* partial_j, double delta, int mode, cudaStream_t st) {
+                         double4* partial, double4* partial_j, double4* acc_j, double delta, int mode, cudaStream_t st) {
     constexpr KernelShape K = kShapeF64Sym;
     if (!p.sym || p.threads != K.threads || p.ipt != K.ipt || p.tile_j != K.tile_j || p.i_begin != 0) {
         set_error("launch_force_sym_f64: not a symmetric FP64 plan");
@@ -238,11 +256,11 @@ int launch_force_sym_f64(const Plan& p, const double* packed, const double* tile
     const double eps2 = delta * delta;
     const bool guard = !(eps2 >= kTinyR2F64);
     if (mode == MODE_FORCE)
-        return guard ? launch_mg<MODE_FORCE, true>(p, packed, tile_mass, block_mass, partial, partial_j, eps2, st)
-                     : launch_mg<MODE_FORCE, false>(p, packed, tile_mass, block_mass, partial, partial_j, eps2, st);
+        return guard ? launch_mg<MODE_FORCE, true>(p, packed, tile_mass, block_mass, partial, partial_j, acc_j, eps2, st)
+                     : launch_mg<MODE_FORCE, false>(p, packed, tile_mass, block_mass, partial, partial_j, acc_j, eps2, st);
     if (mode == MODE_FORCE_POT)
-        return guard ? launch_mg<MODE_FORCE_POT, true>(p, packed, tile_mass, block_mass, partial, partial_j, eps2, st)
-                     : launch_mg<MODE_FORCE_POT, false>(p, packed, tile_mass, block_mass, partial, partial_j, eps2, st);
+        return guard ? launch_mg<MODE_FORCE_POT, true>(p, packed, tile_mass, block_mass, partial, partial_j, acc_j, eps2, st)
+                     : launch_mg<MODE_FORCE_POT, false>(p, packed, tile_mass, block_mass, partial, partial_j, acc_j, eps2, st);
     set_error("launch_force_sym_f64: mode %d has no symmetric kernel", mode);
     return PP_EINVAL;
 }

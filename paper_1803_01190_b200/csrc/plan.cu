@@ -3,11 +3,12 @@
 // The all-pairs sweep of eq. (1) is cut into (i-block, j-split) work units.  The paper's Kepler GPUs
 // had 13-15 SMs, so "one thread per i-particle" filled them at any N of interest; a B200 has 148 SMs
 // and N = 2^20 bodies in 1792-body i-blocks are only 3.96 waves.  The plan therefore picks the shape class (large /
-// mid / small, ppgrav_internal.h) and the split factor S that minimise
+// mid / small, ppgrav_internal.h; by calibrated size thresholds) and the split factor S that minimises
 //     waves x (tiles per split + fixed overhead) x tile cost  +  weight x S x bodies
-// so that the last wave is nearly full.  The class efficiencies and the weight are calibrated on the B200 with the
+// so that the last wave is nearly full.  The class thresholds and the weight are calibrated on the B200 with the
 // throughput-vs-N sweep of `bench.py --sweep-n` (raw data profiles/r2_sweep_n.json).
 #include <algorithm>
+#include <cmath>
 
 #include "ppgrav_internal.h"
 
@@ -15,8 +16,21 @@ namespace ppgrav {
 
 namespace {
 
-// relative pair throughput of one SM running a class (large = 1), per precision; BASELINE.md section 4.2
-constexpr double kClassEff[2][kNumClasses] = {
+// Which shape class serves a solve of i_count i-bodies against N j-bodies: calibrated on the B200 with
+// `bench.py --sweep-n` (profiles/r2_sweep_n.json), where every class was pinned in turn at
+// N = 2^11 .. 2^21.  The fastest class (whole pp_forces call, force only) was
+//   FP32: small up to 2^13, mid at 2^14, large from 2^15;     FP64: small up to 2^14, large from 2^15
+// (the FP64 mid class never beat both neighbours; it stays reachable through PP_CFG_SHAPE).  A range solve is placed by
+// the geometric mean of its two sides.
+int calibrated_class(int precision, int64_t N, int64_t i_count) {
+    const double n_eff = std::sqrt((double)N * (double)i_count);
+    if (precision == PP_F64) return n_eff < 24000.0 ? CLS_SMALL : CLS_LARGE;
+    return n_eff < 12000.0 ? CLS_SMALL : n_eff < 24000.0 ? CLS_MID : CLS_LARGE;
+}
+
+// relative cost of a tile in a class (large = 1), used only to weigh a class's sweep against its partial-sum traffic
+// when S is chosen: the values S was calibrated with in round 1
+constexpr double kClassWeight[2][kNumClasses] = {
     /* PP_F32 */ {1.0, 0.90, 0.45},
     /* PP_F64 */ {1.0, 0.93, 0.80},
 };
@@ -37,8 +51,8 @@ Plan make_plan(int64_t N, int precision, int mode, int sm_count, int64_t forced_
     double best_cost = -1.0;
     const int pi = precision == PP_F64 ? 1 : 0;
     const size_t elem = precision == PP_F64 ? 32 : 16;
-    for (int c = 0; c < kNumClasses; ++c) {
-        if (forced_cls >= 0 && forced_cls < kNumClasses && c != forced_cls) continue;
+    const int cls = (forced_cls >= 0 && forced_cls < kNumClasses) ? forced_cls : calibrated_class(precision, N, i_count);
+    for (int c = cls; c <= cls; ++c) {
         const KernelShape& d = kShapes[pi][c][mode];
         Plan p{};
         p.cls = c;
@@ -63,7 +77,7 @@ Plan make_plan(int64_t N, int precision, int mode, int sm_count, int64_t forced_
                                           std::max<int64_t>(1, (int64_t)((1ull << 30) / (p.part_stride * elem))));
         int64_t s_lo = 1, s_hi = s_max;
         if (forced_split >= 1) s_lo = s_hi = std::min<int64_t>(forced_split, p.n_tiles);
-        const double tile_cost = (double)p.i_per_cta * p.tile_j * d.ctas_per_sm / kClassEff[pi][c];
+        const double tile_cost = (double)p.i_per_cta * p.tile_j * d.ctas_per_sm / kClassWeight[pi][c];
         for (int64_t S = s_lo; S <= s_hi; ++S) {
             const int64_t units = (int64_t)p.n_iblocks * S;
             const int64_t waves = (units + resident - 1) / resident;
@@ -80,7 +94,8 @@ Plan make_plan(int64_t N, int precision, int mode, int sm_count, int64_t forced_
     return best;
 }
 
-Plan make_sym_plan(int64_t N, int precision, int mode, int sm_count, int64_t forced_split, size_t* jbytes) {
+Plan make_sym_plan(int64_t N, int precision, int mode, int sm_count, int64_t forced_split, size_t rows_cap_bytes,
+                   size_t* jbytes, size_t* abytes) {
     const KernelShape& d = precision == PP_F64 ? kShapeF64Sym : kShapeF32Sym;
     const size_t elem = precision == PP_F64 ? 32 : 16;
     Plan p{};
@@ -116,7 +131,14 @@ Plan make_sym_plan(int64_t N, int precision, int mode, int sm_count, int64_t for
                             kFinalizeCost * (double)S * (double)p.part_stride;
         if (best < 0.0 || cost < best * (1.0 - 1e-9)) { best = cost; p.split = (int)S; }
     }
-    if (jbytes) *jbytes = (size_t)p.sym_h * (size_t)p.part_stride * elem;
+    // bands: as many partner offsets per band as rows_cap_bytes holds
+    const size_t row_bytes = (size_t)p.part_stride * elem;
+    p.sym_rows = (int)std::max<size_t>(1, std::min<size_t>((size_t)std::max(p.sym_h, 1), rows_cap_bytes / row_bytes));
+    p.sym_bands = std::max(1, (p.sym_h + p.sym_rows - 1) / p.sym_rows);
+    // every band keeps its own S i-side partials: a banded solve (N > 2^21: thousands of blocks) needs no split-j
+    if (p.sym_bands > 1 && forced_split < 1) p.split = 1;
+    if (jbytes) *jbytes = std::max<size_t>((size_t)std::min(p.sym_rows, std::max(p.sym_h, 1)) * row_bytes, 16);
+    if (abytes) *abytes = p.sym_bands > 1 ? 2 * row_bytes : 0;
     return p;
 }
 

@@ -13,6 +13,12 @@ void set_error(const char* fmt, ...);
 int cuda_fail(cudaError_t e, const char* what);   // records the message, returns PP_ECUDA
 void count_launch(int n = 1);
 
+#define PP_TRY_RC(expr)                 \
+    do {                                \
+        const int rc__ = (expr);        \
+        if (rc__ != PP_OK) return rc__; \
+    } while (0)
+
 #define PP_CUDA(call)                                            \
     do {                                                         \
         cudaError_t e__ = (call);                                \
@@ -102,8 +108,26 @@ constexpr KernelShape kShapeF64Mid = {PP_F64_MID_THREADS, PP_F64_MID_IPT, PP_F64
 constexpr KernelShape kShapeF64Small = {128, 1, 128, 4, 4};
 // shape of the symmetric (every unordered pair once) sweeps: the block must be a whole number of tiles and a tile has
 // one body per thread (its j-side sums are reduced one thread per body)
-constexpr KernelShape kShapeF32Sym = {256, 7, 256, 4, 1};
-constexpr KernelShape kShapeF64Sym = {256, 6, 256, 4, 1};
+#ifndef PP_SYM32_IPT
+#define PP_SYM32_IPT 8
+#endif
+#ifndef PP_SYM32_JP
+#define PP_SYM32_JP 1
+#endif
+#ifndef PP_SYM32_UNROLL
+#define PP_SYM32_UNROLL 2
+#endif
+#ifndef PP_SYM64_IPT
+#define PP_SYM64_IPT 8
+#endif
+#ifndef PP_SYM64_UNROLL
+#define PP_SYM64_UNROLL 2
+#endif
+constexpr int kSymF32Jp = PP_SYM32_JP;          // j-pairs a lane keeps in flight (force_sym_f32.cu)
+constexpr int kSymF32Unroll = PP_SYM32_UNROLL;  // systolic steps per unrolled loop body
+constexpr int kSymF64Unroll = PP_SYM64_UNROLL;
+constexpr KernelShape kShapeF32Sym = {256, PP_SYM32_IPT, 256, 4, 1};
+constexpr KernelShape kShapeF64Sym = {256, PP_SYM64_IPT, 256, 4, 1};
 constexpr KernelShape kShapes[2][kNumClasses][kNumModes] = {
     {{kShapeF32Large, kShapeF32Large, kShapeF32Large},
      {kShapeF32Mid, kShapeF32Mid, kShapeF32Mid},
@@ -138,13 +162,18 @@ struct Plan {
     // symmetric sweep (force_sym_*.cu): every unordered pair once.  Blocks = i-blocks; block I sweeps the blocks
     // I+1 .. I+sym_h two-sidedly; j-side sums go to partial_j[sym_h][part_stride].
     int sym;            // 1 = this plan runs the symmetric kernel
-    int sym_h;          // floor((n_iblocks - 1) / 2)
+    int sym_h;          // floor((n_iblocks - 1) / 2): partner offsets d = 1 .. sym_h
+    int sym_rows;       // partner offsets per band (= rows of partial_j); sym_h when one band holds them all
+    int sym_bands;      // ceil(sym_h / sym_rows), at least 1
 };
 // forced_split >= 1 pins S (capped by the tile count); forced_cls in {0,1,2} pins the shape class, -1 = choose.
 Plan make_plan(int64_t N, int precision, int mode, int sm_count, int64_t forced_split, int forced_cls,
                int64_t i_begin = 0, int64_t i_count = -1);
 // plan of the symmetric sweep for a full solve of N bodies; bytes of its j-side workspace in *jbytes
-Plan make_sym_plan(int64_t N, int precision, int mode, int sm_count, int64_t forced_split, size_t* jbytes);
+// (rows_cap_bytes: the j-side rows of one band may take that much; *jbytes = bytes of partial_j, *abytes = bytes of
+// the running j-side sums acc_j that bands need, 0 for a single band)
+Plan make_sym_plan(int64_t N, int precision, int mode, int sm_count, int64_t forced_split, size_t rows_cap_bytes,
+                   size_t* jbytes, size_t* abytes);
 
 // ---- kernels (one launcher per translation unit) -----------------------------------------------------------------
 // Packed bodies.  FP32: pairs of bodies interleaved, 8 floats {x0 x1 y0 y1 z0 z1 m0 m1} per pair (so that one
@@ -181,10 +210,13 @@ int launch_force_f32(const Plan& p, const float* packed, const float* tile_mass,
                      double delta, int mode, cudaStream_t st);
 // symmetric sweep: i-side sums to partial[S][part_stride], j-side sums to partial_j[sym_h][part_stride] (same sign
 // convention, ready to be added); block_mass[I] = common mass of i-block I or NaN (launch_tile_mass_* with tile = block)
+// With p.sym_bands > 1 the rows are reused band after band and summed into acc_j[2][part_stride] (TwoSum value / error).
 int launch_force_sym_f32(const Plan& p, const float* packed, const float* tile_mass, const float* block_mass,
-                         float4* partial, float4* partial_j, double delta, int mode, cudaStream_t st);
+                         float4* partial, float4* partial_j, float4* acc_j, double delta, int mode, cudaStream_t st);
+int launch_fold_rows(const float4* rows, int nrows, int64_t stride, float4* acc_j, bool first, cudaStream_t st);
+int launch_fold_rows(const double4* rows, int nrows, int64_t stride, double4* acc_j, bool first, cudaStream_t st);
 int launch_force_sym_f64(const Plan& p, const double* packed, const double* tile_mass, const double* block_mass,
-                         double4* partial, double4* partial_j, double delta, int mode, cudaStream_t st);
+                         double4* partial, double4* partial_j, double4* acc_j, double delta, int mode, cudaStream_t st);
 // MODE_POT writes {pot_hi, pot_lo, 0, 0} (double-double partial of the potential sum).
 int launch_force_f64(const Plan& p, const double* packed, const double* tile_mass, double4* partial, int64_t N,
                      double delta, int mode, cudaStream_t st);

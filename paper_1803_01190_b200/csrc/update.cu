@@ -119,6 +119,27 @@ finalize_kernel(const typename Vec4<TP>::type* __restrict__ partial, int split, 
     }
 }
 
+// Symmetric sweep in bands (force_sym_*.cu): acc_j[0][i] + acc_j[1][i] (TwoSum value and error) += sum_r rows[r][i],
+// in row order -- the j-side sums of one band of partner offsets, so that the rows can be reused by the next band.
+template <typename T4, typename T>
+__global__ void __launch_bounds__(kThreads)
+fold_rows_kernel(const T4* __restrict__ rows, int nrows, int64_t stride, T4* __restrict__ acc_j, int first) {
+    const int64_t i = (int64_t)blockIdx.x * kThreads + threadIdx.x;
+    if (i >= stride) return;
+    T4 s, c;
+    if (first) { s.x = s.y = s.z = s.w = 0; c = s; }
+    else { s = acc_j[i]; c = acc_j[stride + i]; }
+    for (int r = 0; r < nrows; ++r) {
+        const T4 v = rows[(size_t)r * stride + i];
+        comp_add(s.x, c.x, v.x);
+        comp_add(s.y, c.y, v.y);
+        comp_add(s.z, c.z, v.z);
+        comp_add(s.w, c.w, v.w);
+    }
+    acc_j[i] = s;
+    acc_j[stride + i] = c;
+}
+
 // TK: scalar type of the packed copy (the sweep's precision; float for a double state in PP_MIXED)
 template <typename T, typename TK>
 __global__ void __launch_bounds__(kThreads)
@@ -196,6 +217,19 @@ kick_drift_kernel(T* __restrict__ pos, T* __restrict__ vel, const T* __restrict_
 }
 
 }  // namespace
+
+int launch_fold_rows(const float4* rows, int nrows, int64_t stride, float4* acc_j, bool first, cudaStream_t st) {
+    fold_rows_kernel<float4, float><<<grid_for(stride), kThreads, 0, st>>>(rows, nrows, stride, acc_j, first ? 1 : 0);
+    count_launch();
+    PP_CUDA(cudaGetLastError());
+    return PP_OK;
+}
+int launch_fold_rows(const double4* rows, int nrows, int64_t stride, double4* acc_j, bool first, cudaStream_t st) {
+    fold_rows_kernel<double4, double><<<grid_for(stride), kThreads, 0, st>>>(rows, nrows, stride, acc_j, first ? 1 : 0);
+    count_launch();
+    PP_CUDA(cudaGetLastError());
+    return PP_OK;
+}
 
 int launch_kick_drift_f32(float* pos, float* vel, const float* acc, int64_t n, double kick, double dt,
                           cudaStream_t st) {

@@ -18,6 +18,7 @@ import numpy as np
 PP_F32, PP_F64, PP_MIXED = 0, 1, 2
 PP_ACC_VALID = 1
 PP_CFG_SPLIT_J, PP_CFG_GRAPH, PP_CFG_PROFILE, PP_CFG_EQUAL_MASS, PP_CFG_SHAPE, PP_CFG_SYMMETRIC = 1, 2, 3, 4, 5, 6
+PP_CFG_SYM_BAND_ROWS = 7
 SHAPE_AUTO, SHAPE_LARGE, SHAPE_MID, SHAPE_SMALL = 0, 1, 2, 3
 INVARIANT_NAMES = ("E", "K", "W", "Px", "Py", "Pz", "Lx", "Ly", "Lz", "Cx", "Cy", "Cz", "M")
 
@@ -124,7 +125,8 @@ def pp_plan_query(N, precision, with_pot=False):
     out = (ctypes.c_int64 * 16)()
     _check(lib().pp_plan_query(int(N), int(precision), int(bool(with_pot)), out), "pp_plan_query")
     keys = ("i_per_cta", "tile_j", "split", "ctas", "ctas_per_sm", "sm_count", "pipe_ops_per_evaluation",
-            "mufu_per_evaluation", "shape", "threads", "ipt", "i_blocks", "pairs_per_evaluation", "sym_partner_blocks")
+            "mufu_per_evaluation", "shape", "threads", "ipt", "i_blocks", "pairs_per_evaluation", "sym_partner_blocks",
+            "sym_bands")
     d = dict(zip(keys, (int(v) for v in out)))
     # per ordered pair (pair interaction): what the roofline counts; one less on equal-mass tiles
     d["pipe_ops_per_pair"] = d["pipe_ops_per_evaluation"] / d["pairs_per_evaluation"]

@@ -43,7 +43,7 @@ SHAPES = {0: {"large": (1792, 512), "mid": (512, 256), "small": (128, 128)},
 
 @pytest.mark.parametrize("prec", [0, 1])
 def test_plan_is_sane(ppgrav, prec):
-    allowed_i = {v[0] for v in SHAPES[prec].values()} | ({1792} if prec else set())   # FP64 force-only: 7 per thread
+    allowed_i = {v[0] for v in SHAPES[prec].values()} | {1792, 2048}   # FP64 force-only: 7 per thread; symmetric: 8
     allowed_t = {v[1] for v in SHAPES[prec].values()} | {256}                          # symmetric sweeps: 256
     for n in (1, 2, 100, 2048, 2 ** 14, 2 ** 17, 2 ** 20, 2 ** 22, 2 ** 23):
         for with_pot in (False, True):
@@ -58,26 +58,32 @@ def test_plan_is_sane(ppgrav, prec):
             elem = 32 if prec else 16
             assert p["split"] * n_ib * p["i_per_cta"] * elem <= (1 << 30) or p["split"] == 1
             if p["shape"] == 3:                    # symmetric sweep: one evaluation serves two ordered pairs
-                assert (p["i_per_cta"], p["tile_j"]) == ((1536, 256) if prec else (1792, 256))
+                assert (p["i_per_cta"], p["tile_j"]) == (2048, 256)
                 assert p["pairs_per_evaluation"] == 2 and p["sym_partner_blocks"] == (n_ib - 1) // 2
                 assert p["pipe_ops_per_pair"] == ((11.5 if with_pot else 10) if prec else (9 if with_pot else 8))
             else:
                 assert p["pipe_ops_per_pair"] == ((18 if with_pot else 16) if prec else (13 if with_pot else 12))
-    # calibrated choices: the throughput shape from N = 2^17 up, the mid shape around 2^14,
-    # one body per thread for tiny systems
+    # calibrated choices: one body per thread for small systems, the mid class at 2^14 (FP32),
+    # the large one-sided class at 2^15 and above 2^21, the symmetric sweep from 2^16 to 2^21
     for n in (2 ** 17, 2 ** 20, 2 ** 23):
         p = ppgrav.pp_plan_query(n, prec)
-        # full solves up to 2^21 take the symmetric sweep (its j-side workspace must stay under 48 GB)
-        assert p["shape"] == (3 if n <= 2 ** 21 else 0) and p["i_per_cta"] >= 1536
-    for n in (100, 1024):
+        # full solves take the symmetric sweep; beyond 2^21 its j-side rows (> 48 GB) are worked through in bands
+        assert p["shape"] == 3 and p["i_per_cta"] >= 1536 and (p["sym_bands"] == 1) == (n <= 2 ** 21)
+        elem = 32 if prec else 16
+        rows = -(-p["sym_partner_blocks"] // p["sym_bands"])
+        assert rows * p["i_blocks"] * p["i_per_cta"] * elem <= (16 if p["sym_bands"] > 1 else 48) << 30
+    for n in (100, 1024, 2 ** 13):
         assert ppgrav.pp_plan_query(n, prec)["shape"] == 2
+    assert ppgrav.pp_plan_query(2 ** 14, prec)["shape"] == (2 if prec else 1)
+    assert ppgrav.pp_plan_query(2 ** 15, prec)["shape"] == 0 and ppgrav.pp_plan_query(2 ** 16, prec)["shape"] == 3
     # FP64 per-mode shapes of the large class share the tile size (so they share tile masses and padding rules)
-    if prec:
-        f, fp = ppgrav.pp_plan_query(2 ** 23, 1, False), ppgrav.pp_plan_query(2 ** 23, 1, True)
-        assert (f["ipt"], fp["ipt"]) == (7, 6) and f["tile_j"] == fp["tile_j"]
     ppgrav.pp_configure(ppgrav.PP_CFG_SYMMETRIC, 0)
     try:
         big = ppgrav.pp_plan_query(2 ** 20, prec, True)
+        assert big["shape"] == 0
+        if prec:
+            f, fp = ppgrav.pp_plan_query(2 ** 20, 1, False), big
+            assert (f["ipt"], fp["ipt"]) == (7, 6) and f["tile_j"] == fp["tile_j"]
     finally:
         ppgrav.pp_configure(ppgrav.PP_CFG_SYMMETRIC, 1)
     resident = big["sm_count"] * big["ctas_per_sm"]

@@ -225,7 +225,7 @@ def test_forces_range_eighths_of_2p17_on_the_large_shape(gpu, oracle, prec):
     rng = np.random.Generator(np.random.Philox(key=5))
     with _Pinned(gpu, "large", 2) as pin:
         full_plan = pin.check(n, prec, True)
-        assert sum(1 for k in range(8) if (k * (n // 8)) % full_plan["i_per_cta"]) >= 6   # starts off the block grid
+        assert sum(1 for k in range(8) if (k * (n // 8)) % full_plan["i_per_cta"]) >= 5   # starts off the block grid
         a_full, p_full = gpu.pp_forces(dpos, dmass, delta=c["delta"], want_pot=True)
         for k in range(8):
             b, cnt = k * (n // 8), n // 8
@@ -257,7 +257,7 @@ def test_mixed_precision_on_pinned_shapes(gpu, oracle, shape):
 @pytest.mark.parametrize("prec", ["f64", "f32", "mixed"])
 def test_five_step_trajectory_at_2p15_on_the_large_shape(gpu, oracle, prec):
     """pp_step_kdk against oracle.kdk_halfkick step for step on the kernels the bench times: config 1's recipe (disk +
-    halo, two mass species) at N = 2^15, 5 steps, large class pinned (the plan would take the mid class at this N).
+    halo, two mass species) at N = 2^15, 5 steps, large class pinned.
     Final r, v of ALL bodies within DESIGN.md section 6's trajectory tolerances; a(t_end) and Phi(t_end) too."""
     import torch
     from paper_1803_01190_b200 import workloads
@@ -314,7 +314,10 @@ def test_invariants_potential_sweep_equal_mass_shortcut(gpu, oracle, prec):
                 outs[(shape, flag)] = out
     finally:
         gpu.pp_configure(gpu.PP_CFG_EQUAL_MASS, 1)
-    assert outs[("large", 1)][2] != outs[("large", 0)][2] or outs[("mid", 1)][2] != outs[("mid", 0)][2]
+    # (the double-double tile folding makes W of the two paths agree to the last bits; that the shortcut path exists
+    # on these masses is what pp_equal_mass_tiles reports)
+    n_tiles, n_common = gpu.pp_equal_mass_tiles(dmass)
+    assert n_common >= n_tiles - 4 and abs(outs[("large", 1)][2] - outs[("large", 0)][2]) <= 1e-14 * abs(ref["raw"][2])
 
 
 def test_default_stream_replays_the_step_graph(gpu):
@@ -379,9 +382,9 @@ class _Symmetric:
 
 
 # one block; two blocks (even: no symmetric partner, the opposite block one-sided); three (odd, H = 1); four (H = 1 and
-# the opposite block); five, six, nine blocks; ragged tails just around the 1792-body block and 256-body tile edges
-# (block = 1792 bodies in FP32, 1536 in FP64)
-SYM_N = [1, 2, 255, 1535, 1537, 1791, 1793, 3073, 3585, 4609, 5377, 6145, 7169, 8961, 9217, 15000]
+# the opposite block); five, six, seven, eight, ten blocks; ragged tails just around the block and 256-body tile edges
+# (block = 2048 bodies)
+SYM_N = [1, 2, 255, 2047, 2049, 4097, 6145, 8193, 10241, 12289, 15000, 18433]
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32", "mixed"])
@@ -397,7 +400,7 @@ def test_symmetric_sweep_edge_sizes(gpu, oracle, prec, n):
         for split in (0, 1, 3):
             with _Symmetric(gpu, split):
                 plan = gpu.pp_plan_query(n, gpu.PP_F64 if prec == "f64" else gpu.PP_F32, True)
-                assert plan["shape"] == 3 and plan["i_per_cta"] == (1536 if prec == "f64" else 1792) and plan["tile_j"] == 256
+                assert plan["shape"] == 3 and plan["i_per_cta"] == 2048 and plan["tile_j"] == 256
                 acc, pot = gpu.pp_forces(dpos, dmass, G=2.5, delta=0.05, want_pot=True, mixed=(prec == "mixed"))
                 acc2, _ = gpu.pp_forces(dpos, dmass, G=2.5, delta=0.05, want_pot=False, mixed=(prec == "mixed"))
             if n == 1:
@@ -415,7 +418,7 @@ def test_symmetric_sweep_delta_zero_and_bitwise_reproducible(gpu, oracle, prec, 
     n = 9001
     pos, _, mass = _cloud(n, 93, masses)
     pos, mass = _seen(prec, pos, mass)
-    a, b = 7, 6000                       # a coincident pair in two different blocks: met in a symmetric tile
+    a, b = 7, 6000                       # a coincident pair in two different 2048-body blocks: met in a symmetric tile
     pos[b] = pos[a]
     dpos, dmass = _dev(prec, pos, mass)
     with _Symmetric(gpu):
@@ -436,6 +439,45 @@ def test_symmetric_sweep_delta_zero_and_bitwise_reproducible(gpu, oracle, prec, 
     a_ref[keep != a] += mass[b] * d / r2[:, None] ** 1.5
     p_ref[keep != a] -= mass[b] / np.sqrt(r2)
     assert _rel(acc[keep], a_ref) <= TOL[prec] and _rel(pot[keep], p_ref) <= TOL[prec]
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32", "mixed"])
+@pytest.mark.parametrize("band_rows", [1, 2])
+def test_symmetric_sweep_in_bands(gpu, oracle, prec, band_rows):
+    """Beyond N = 2^21 the j-side rows no longer fit the workspace at once and the partner offsets are worked through
+    in bands (rows reused, folded into running sums in between).  PP_CFG_SYM_BAND_ROWS pins 1 or 2 offsets per band at
+    N = 15000 (8 blocks, H = 3: 3 bands of one offset, or 2 bands the second of which is ragged); all bodies against
+    the oracle, forced split-j 1 and 3, a 3-step trajectory, and bit-identical run to run."""
+    import torch
+    n = 15000
+    seen = "f64" if prec == "f64" else "f32"
+    pos, vel, mass = _cloud(n, 7000 + n, "species")
+    ps, vs, ms = _seen(seen, pos, vel, mass)
+    a_ref, p_ref = _oracle_forces(oracle, (n, "sym" + seen, "species"), ps, ms, 2.5, 0.05)
+    st = "f32" if prec == "f32" else "f64"
+    dpos, dvel, dmass = _dev(st, *((ps, vs, ms) if prec != "mixed" else (pos, vel, mass)))
+    mixed = prec == "mixed"
+    gpu.pp_configure(gpu.PP_CFG_SYM_BAND_ROWS, band_rows)
+    try:
+        for split in (1, 3):
+            with _Symmetric(gpu, split):
+                plan = gpu.pp_plan_query(n, gpu.PP_F64 if prec == "f64" else gpu.PP_F32, True)
+                assert plan["shape"] == 3 and plan["sym_bands"] == -(-plan["sym_partner_blocks"] // band_rows) >= 2
+                acc, pot = gpu.pp_forces(dpos, dmass, G=2.5, delta=0.05, want_pot=True, mixed=mixed)
+                acc2, _ = gpu.pp_forces(dpos, dmass, G=2.5, delta=0.05, mixed=mixed)
+                acc3, pot3 = gpu.pp_forces(dpos, dmass, G=2.5, delta=0.05, want_pot=True, mixed=mixed)
+            assert torch.equal(acc, acc3) and torch.equal(pot, pot3)
+            assert _rel(acc.cpu().numpy(), a_ref) <= TOL[seen] and _rel(acc2.cpu().numpy(), a_ref) <= TOL[seen]
+            assert _rel(pot.cpu().numpy(), p_ref) <= TOL[seen]
+        if prec != "mixed":
+            p3, v3, _, _ = oracle.kdk_halfkick(ps, vs, ms, 1e-3, 3, G=2.5, delta=0.05, nthreads=0)
+            dacc = torch.zeros_like(dpos)
+            with _Symmetric(gpu):
+                gpu.pp_step_kdk(dpos, dvel, dmass, dacc, 1e-3, 3, G=2.5, delta=0.05)
+            assert np.abs(dpos.cpu().numpy() - p3).max() / np.abs(p3).max() <= TOL_TRAJ[seen]
+            assert np.abs(dvel.cpu().numpy() - v3).max() / np.abs(v3).max() <= TOL_TRAJ[seen]
+    finally:
+        gpu.pp_configure(gpu.PP_CFG_SYM_BAND_ROWS, 0)
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])

@@ -195,9 +195,11 @@ def test_sharded_step_equals_single_gpu_step(gpu, oracle, prec, world, n):
     P = sum(p[3:6] for p in parts)
     M = sum(p[12] for p in parts)
     com = sum(p[9:12] * p[12] for p in parts) / M
-    assert abs(E - whole["E"]) <= 1e-12 * abs(whole["E"])
-    assert np.abs(P - whole["P"]).max() <= 1e-14 * float(np.sum(mass[:, None] * np.abs(vel)))
-    assert abs(M - whole["M"]) <= 1e-14 * M and np.abs(com - whole["COM"]).max() <= 1e-13
+    # (world does not divide N: the shards' potentials differ from the whole-system ones by summation-order round-off)
+    loose = 1.0 if n % world == 0 or prec == "f64" else 1e6       # FP32 states that differ by FP32 round-off
+    assert abs(E - whole["E"]) <= 1e-12 * loose * abs(whole["E"])
+    assert np.abs(P - whole["P"]).max() <= 1e-14 * loose * float(np.sum(mass[:, None] * np.abs(vel)))
+    assert abs(M - whole["M"]) <= 1e-14 * M and np.abs(com - whole["COM"]).max() <= 1e-13 * loose
 
 
 def test_sharded_system_world1_invariants(gpu):
