@@ -38,8 +38,9 @@ UNIT = "pair-interactions/s"
 # nominal pipe peaks: lanes per SM x SMs x max SM clock
 FP32_LANES, FP64_LANES, SM_COUNT, SM_MAX_HZ = 128, 64, 148, 1.965e9
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE sweep launch (with potential) at N = 2^20, from the
-# `ncu --set full` captures summarised in profiles/r1d_force_f32_ncu.md / profiles/r1d_force_f64_ncu.md
-NCU_TRAFFIC_BYTES = {("f32", 1 << 20): 17.038848e6 + 0.0, ("f64", 1 << 20): 68.253184e6 + 106.742784e6}
+# `ncu --set full` captures summarised in profiles/r2_force_sym_f32_ncu.md / profiles/r2_force_sym_f64_ncu.md (the
+# symmetric sweeps: the writes are their j-side rows, N^2/(2 x 2048) x 16 or 32 B, written once)
+NCU_TRAFFIC_BYTES = {("f32", 1 << 20): 136.68864e6 + 4267.070e6, ("f64", 1 << 20): 381.68704e6 + 8597.523e6}
 L2_FLUSH_BYTES = 256 << 20
 
 
@@ -172,6 +173,7 @@ def run_ours(args):
         flush_buf.zero_()                              # > 126 MB L2: the next step starts cold
 
     results = {}
+    gpu_samples = {}
     clocks = None
     launches = None
     precisions = [("f32", torch.float32)] + ([] if args.no_fp64 else [("f64", torch.float64)])
@@ -231,7 +233,16 @@ def run_ours(args):
                                       (lanes, "FP32" if name == "f32" else "FP64", SM_COUNT, SM_MAX_HZ / 1e6)),
             plan=plan, E_after=inv["E"])
 
-        # force-only single evaluation (12 / 16 pipe operations per pair)
+        # parity sample for the cpu_baseline leg: accelerations and potentials of 4096 sampled bodies of the ORIGINAL
+        # inputs from the same launch configuration (untimed)
+        if world == 1 and not args.no_cpu_baseline:
+            idx_t = torch.tensor(workloads.sample_indices(c["seed"], N, 4096), device="cuda")
+            pos0 = torch.tensor(c["pos"], dtype=dtype, device="cuda")
+            a0, p0 = ppgrav.pp_forces(pos0, mass, G=G, delta=delta, want_pot=True)
+            gpu_samples[name] = (a0[idx_t].double().cpu().numpy(), p0[idx_t].double().cpu().numpy())
+            del pos0, a0, p0
+
+        # force-only single evaluation
         def force_only():
             ppgrav.pp_forces(pos, mass, G=G, delta=delta, acc=acc)
 
@@ -308,7 +319,7 @@ def run_ours(args):
             line["kdk_step"] = {"config0": kdk_step_latency(torch, ppgrav, workloads, 0, 10),
                                 "config1": kdk_step_latency(torch, ppgrav, workloads, 1, 20, reps=2)}
         if world == 1 and not args.no_cpu_baseline:
-            line["cpu_baseline"] = cpu_baseline(c, n_sample=16384)
+            line["cpu_baseline"] = cpu_baseline(c, n_sample=16384, gpu_samples=gpu_samples)
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
@@ -500,8 +511,10 @@ def run_sharded(args):
 
 
 # ---- the oracle on the host cores --------------------------------------------------------------------------------
-def cpu_baseline(c, n_sample):
-    """Times oracle.forces (as it stands) on a bounded sample of i-bodies against all N j-bodies."""
+def cpu_baseline(c, n_sample, gpu_samples=None):
+    """Times oracle.forces (as it stands) on a bounded sample of i-bodies against all N j-bodies, and -- untimed --
+    compares the GPU's accelerations / potentials of 4096 sampled bodies (same launch configuration as the timed
+    steps) with the oracle's: max over the sample of |a_gpu - a_oracle| / |a_oracle| (BASELINE.json's parity metric)."""
     from oracle import oracle
     from paper_1803_01190_b200 import workloads
     idx = workloads.sample_indices(c["seed"], c["N"], n_sample)
@@ -515,7 +528,16 @@ def cpu_baseline(c, n_sample):
     t0 = time.perf_counter()
     oracle.forces(c["pos"], c["mass"], G=c["G"], delta=c["delta"], idx=idx1, want_pot=True, nthreads=1)
     sec1 = time.perf_counter() - t0
+    parity = {}
+    for name, (ga, gp) in (gpu_samples or {}).items():
+        pidx = workloads.sample_indices(c["seed"], c["N"], 4096)
+        pos, mass = (c["pos"], c["mass"]) if name == "f64" else workloads.as_f32_exact(c["pos"], c["mass"])
+        ra, rp = oracle.forces(pos, mass, G=c["G"], delta=c["delta"], idx=pidx, want_pot=True, nthreads=0)
+        parity[name] = {"max_rel_err_acc": float(np.max(np.linalg.norm(ga - ra, axis=1) / np.linalg.norm(ra, axis=1))),
+                        "max_rel_err_pot": float(np.max(np.abs(gp - rp) / np.abs(rp))), "sampled_bodies": int(len(pidx)),
+                        "tolerance": 1e-12 if name == "f64" else 2e-5}
     return {"value": pairs / sec, "unit": UNIT, "cores": cores, "kind": "oracle", "seconds": sec,
+            "parity_vs_oracle": parity,
             "single_thread_value": float(len(idx1)) * float(c["N"] - 1) / sec1, "single_thread_seconds": sec1,
             "sample": "oracle.forces (FP64, compensated sums, OpenMP over i) for %d sampled i-bodies x all %d "
                       "j-bodies of the same workload = %.3g pairs; single thread: the first %d of them" %

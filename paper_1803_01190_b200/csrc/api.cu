@@ -284,8 +284,8 @@ bool symmetric_plan(int64_t N, int sweep_prec, int mode, int sm_count, bool full
     if (cfg == 0 || !full || (mode != MODE_FORCE && mode != MODE_FORCE_POT)) return false;
     if (cfg == 1) {   // automatic: not when a shape class is pinned (PP_CFG_SHAPE addresses the one-sided kernels)
         if (forced_class() >= 0) return false;
-        // measured: faster than the large one-sided class from N = 2^16 on, slower at 2^15
-        if (N < 49152 || make_plan(N, sweep_prec, mode, sm_count, 0, -1).cls != CLS_LARGE) return false;
+        // measured: faster than the large one-sided class from N = 2^17 on, slower at 2^16
+        if (N < 98304 || make_plan(N, sweep_prec, mode, sm_count, 0, -1).cls != CLS_LARGE) return false;
     }
     size_t jbytes = 0, abytes = 0;
     Plan sp = make_sym_plan(N, sweep_prec, mode, sm_count, g_cfg_split.load(), kMaxPartialJBytes, &jbytes, &abytes);

@@ -41,6 +41,10 @@ int64_t round_up(int64_t a, int64_t b) { return (a + b - 1) / b * b; }
 // interactions of one SM.  The bandwidth cost alone is ~0.1; the weight is larger so that a bigger S is only taken when
 // it fills the last wave noticeably better.
 constexpr double kFinalizeCost = 16.0;
+// the same for the symmetric sweep, whose tile costs 29 us against ~1.4 us for writing and re-reading one more
+// partial sum per body at N = 2^17: a small weight, so that S = 8-9 fills the 148 SMs at N = 2^17 .. 2^18, where
+// 64-128 blocks alone leave a seventh of them idle
+constexpr double kSymFinalizeCost = 2.0;
 
 }  // namespace
 
@@ -127,8 +131,11 @@ Plan make_sym_plan(int64_t N, int precision, int mode, int sm_count, int64_t for
     for (int64_t S = s_lo; S <= s_hi; ++S) {
         const int64_t units = (int64_t)p.n_iblocks * S;
         const int64_t waves = (units + sm_count - 1) / sm_count;
-        const double cost = (double)waves * ((double)((ptiles + S - 1) / S) + 2.0 * tpb + 2.0) * p.i_per_cta * p.tile_j +
-                            kFinalizeCost * (double)S * (double)p.part_stride;
+        // per unit: its share of the partner tiles + 2 tile-times of fill and epilogue; the one-sided tiles (own block,
+        // and the opposite block when the block count is even) ride on the split-0 units, i.e. once on the critical path
+        const double n_ns = (double)tpb * ((p.n_iblocks > 1 && p.n_iblocks % 2 == 0) ? 2.0 : 1.0);
+        const double cost = ((double)waves * ((double)((ptiles + S - 1) / S) + 2.0) + n_ns) * p.i_per_cta * p.tile_j +
+                            kSymFinalizeCost * (double)S * (double)p.part_stride;
         if (best < 0.0 || cost < best * (1.0 - 1e-9)) { best = cost; p.split = (int)S; }
     }
     // bands: as many partner offsets per band as rows_cap_bytes holds

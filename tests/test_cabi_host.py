@@ -64,7 +64,7 @@ def test_plan_is_sane(ppgrav, prec):
             else:
                 assert p["pipe_ops_per_pair"] == ((18 if with_pot else 16) if prec else (13 if with_pot else 12))
     # calibrated choices: one body per thread for small systems, the mid class at 2^14 (FP32),
-    # the large one-sided class at 2^15 and above 2^21, the symmetric sweep from 2^16 to 2^21
+    # the large one-sided class at 2^15 and 2^16, the symmetric sweep from 2^17
     for n in (2 ** 17, 2 ** 20, 2 ** 23):
         p = ppgrav.pp_plan_query(n, prec)
         # full solves take the symmetric sweep; beyond 2^21 its j-side rows (> 48 GB) are worked through in bands
@@ -75,7 +75,8 @@ def test_plan_is_sane(ppgrav, prec):
     for n in (100, 1024, 2 ** 13):
         assert ppgrav.pp_plan_query(n, prec)["shape"] == 2
     assert ppgrav.pp_plan_query(2 ** 14, prec)["shape"] == (2 if prec else 1)
-    assert ppgrav.pp_plan_query(2 ** 15, prec)["shape"] == 0 and ppgrav.pp_plan_query(2 ** 16, prec)["shape"] == 3
+    assert ppgrav.pp_plan_query(2 ** 15, prec)["shape"] == 0 and ppgrav.pp_plan_query(2 ** 16, prec)["shape"] == 0
+    assert ppgrav.pp_plan_query(2 ** 17, prec)["shape"] == 3
     # FP64 per-mode shapes of the large class share the tile size (so they share tile masses and padding rules)
     ppgrav.pp_configure(ppgrav.PP_CFG_SYMMETRIC, 0)
     try:
