@@ -259,6 +259,24 @@ def run_ours(args):
         ppgrav.pp_configure(ppgrav.PP_CFG_SYMMETRIC, 1)
         results[name]["force_only_one_sided"] = replicas.job_value(pairs, 2, oms, world)
 
+        if name == "f64" and world == 1 and not args.no_kdk_latency:
+            # pp_invariants with its own FP64 potential sweep (pot = NULL; what the conservation experiment pays per
+            # sample): equal-mass shortcut on (11 operations per pair) and off (12)
+            inv_ms = {}
+            for key, flag in (("equal_mass_shortcut", 1), ("shortcut_off", 0)):
+                ppgrav.pp_configure(ppgrav.PP_CFG_EQUAL_MASS, flag)
+                ts = []
+                for r in range(2):
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record()
+                    ppgrav.pp_invariants(pos, vel, mass, G=G, delta=delta, out16=out16)
+                    e1.record()
+                    torch.cuda.synchronize()
+                    ts.append(e0.elapsed_time(e1))
+                inv_ms[key] = ts[-1]
+            ppgrav.pp_configure(ppgrav.PP_CFG_EQUAL_MASS, 1)
+            results[name]["invariants_with_potential_sweep_ms"] = inv_ms
+
         if name == "f32" and not args.no_e2e:
             # end to end through the host-buffer C ABI: pinned host arrays in, results back, every step
             hp, hv, hm, ha, hpot = (torch.empty(s, dtype=dtype).pin_memory().numpy()
@@ -313,7 +331,8 @@ def run_ours(args):
             r64 = results["f64"]
             line["fp64"] = {"value": r64["value"], "unit": UNIT, "ms_per_step": r64["ms_per_step"],
                             "roofline": r64["roofline"], "sweep_ms_per_launch": r64["sweep_ms_per_launch"],
-                            "plan": r64["plan"], "fp64_over_fp32_time": r64["ms_per_step"] / r32["ms_per_step"]}
+                            "plan": r64["plan"], "fp64_over_fp32_time": r64["ms_per_step"] / r32["ms_per_step"],
+                            "invariants_with_potential_sweep_ms": r64.get("invariants_with_potential_sweep_ms")}
         if world == 1 and not args.no_kdk_latency:
             # BASELINE.json's KDK-step configs: 0 (N = 2048, 10 steps per call) and 1 (N = 2^17, 200 steps; 20 per call)
             line["kdk_step"] = {"config0": kdk_step_latency(torch, ppgrav, workloads, 0, 10),

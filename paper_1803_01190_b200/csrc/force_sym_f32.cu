@@ -24,6 +24,9 @@
 //    bit-reproducible run to run.
 //  * Equal-mass shortcut as in force_f32.cu, now needing a common mass on both sides (the j-tile's, applied to the i-side
 //    fold; the i-block's, applied to the j-side reduction).  Otherwise m_j w^3 and m_i w^3 are formed per pair.
+#ifndef PP_SYM32_ORDER
+#define PP_SYM32_ORDER 0
+#endif
 #include "force_f32_common.cuh"
 #include <algorithm>
 
@@ -72,12 +75,21 @@ __device__ __forceinline__ void sym_chunk(float2 (&xj)[JP], float2 (&yj)[JP], fl
                 const float2 w3 = __fmul2_rn(w, __fmul2_rn(w, w));
                 const float2 si = UNI ? w3 : __fmul2_rn(mj[q], w3);  // pull of j on i:  m_j w^3 (r_j - r_i)
                 const float2 sj = UNI ? w3 : __fmul2_rn(mi[k], w3);  // pull of i on j: -m_i w^3 (r_j - r_i), sign in the reduction
+#if PP_SYM32_ORDER == 1   // tuning knob: i-side and j-side update of one component back to back (shared operands)
+                ax[k] = __ffma2_rn(si, dx, ax[k]);
+                fx[q] = __ffma2_rn(sj, dx, fx[q]);
+                ay[k] = __ffma2_rn(si, dy, ay[k]);
+                fy[q] = __ffma2_rn(sj, dy, fy[q]);
+                az[k] = __ffma2_rn(si, dz, az[k]);
+                fz[q] = __ffma2_rn(sj, dz, fz[q]);
+#else
                 ax[k] = __ffma2_rn(si, dx, ax[k]);
                 ay[k] = __ffma2_rn(si, dy, ay[k]);
                 az[k] = __ffma2_rn(si, dz, az[k]);
                 fx[q] = __ffma2_rn(sj, dx, fx[q]);
                 fy[q] = __ffma2_rn(sj, dy, fy[q]);
                 fz[q] = __ffma2_rn(sj, dz, fz[q]);
+#endif
                 if (MODE == MODE_FORCE_POT) {
                     ap[k] = UNI ? __fadd2_rn(ap[k], w) : __ffma2_rn(mj[q], w, ap[k]);
                     fp[q] = UNI ? __fadd2_rn(fp[q], w) : __ffma2_rn(mi[k], w, fp[q]);
