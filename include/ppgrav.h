@@ -139,7 +139,8 @@ int pp_kick_drift(void* pos, void* vel, const void* acc, int64_t n, double kick,
  *   performs no solve (nsteps == 0 with PP_ACC_VALID) pot is left untouched.
  * nsteps == 0 only (re)computes acc.  Force evaluations performed: nsteps (+1 without PP_ACC_VALID).
  * Kernel launches: 1 (tile masses) + 3 for a cold start + 1 (kick+drift+pack) + 2 per interior step boundary
- * (pair sweep, fused update pass) + 2 (last sweep, finalize+kick) = 2 nsteps + 2 (+3).  For N <= 65536 the interior
+ * (pair sweep, fused update pass) + 2 (last sweep, finalize+kick) = 2 nsteps + 2 (+3); the symmetric sweep adds one per
+ * call (block masses) and, beyond N = 2^21, one sweep and one fold launch per band of partner offsets.  For N <= 65536 the interior
  * steps are replayed from a CUDA graph that is kept while the arguments do not change (also when `stream` is the legacy
  * default stream: the replay then runs on an internal stream, ordered with `stream` by events). */
 int pp_step_kdk(void* pos, void* vel, const void* mass, void* acc, void* pot, int64_t N, double dt, int64_t nsteps,

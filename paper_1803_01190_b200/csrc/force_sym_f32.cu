@@ -10,7 +10,8 @@
 //  * Bodies are cut into blocks of B = THREADS x IPT (256 x 8 = 2048).  Block I owns the unordered block pairs (I, I+d),
 //    d = 1 .. H = floor((nb-1)/2), cyclically: every pair of distinct blocks exactly once, the same load for every I.
 //    Its own block (and, for an even number of blocks, the block opposite, I + nb/2, which two CTAs share) is swept the
-//    ordinary one-sided way (sweep_tile of force_f32_common.cuh): B/N of the work.
+//    ordinary one-sided way (sweep_tile of force_f32_common.cuh): B/N of the work.  Split-j cuts the block's whole tile
+//    list -- one-sided tiles first, then the partner tiles -- into S equal parts.
 //  * j-tiles arrive through the same TMA ring as in force_f32.cu.  Inside a tile every lane of a warp takes one j-PAIR
 //    (two bodies, one packed operand) into registers together with a packed accumulator for the pull of the warp's
 //    i-bodies on it; 32 systolic steps rotate the j-pairs (and their accumulators) through the lanes by warp shuffles,
@@ -25,7 +26,7 @@
 //  * Equal-mass shortcut as in force_f32.cu, now needing a common mass on both sides (the j-tile's, applied to the i-side
 //    fold; the i-block's, applied to the j-side reduction).  Otherwise m_j w^3 and m_i w^3 are formed per pair.
 #ifndef PP_SYM32_ORDER
-#define PP_SYM32_ORDER 0
+#define PP_SYM32_ORDER 1   // measured: 267 against 274 ms force-only at N = 2^20 (profiles/r2_sym_tuning.md)
 #endif
 #include "force_f32_common.cuh"
 #include <algorithm>
@@ -75,7 +76,7 @@ __device__ __forceinline__ void sym_chunk(float2 (&xj)[JP], float2 (&yj)[JP], fl
                 const float2 w3 = __fmul2_rn(w, __fmul2_rn(w, w));
                 const float2 si = UNI ? w3 : __fmul2_rn(mj[q], w3);  // pull of j on i:  m_j w^3 (r_j - r_i)
                 const float2 sj = UNI ? w3 : __fmul2_rn(mi[k], w3);  // pull of i on j: -m_i w^3 (r_j - r_i), sign in the reduction
-#if PP_SYM32_ORDER == 1   // tuning knob: i-side and j-side update of one component back to back (shared operands)
+#if PP_SYM32_ORDER == 1   // i-side and j-side update of one component back to back: they share two operands
                 ax[k] = __ffma2_rn(si, dx, ax[k]);
                 fx[q] = __ffma2_rn(sj, dx, fx[q]);
                 ay[k] = __ffma2_rn(si, dy, ay[k]);
@@ -126,16 +127,18 @@ force_sym_f32_kernel(const float* __restrict__ packed, const float* __restrict__
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int I = blockIdx.x;
     const int S = gridDim.y, sidx = blockIdx.y;
-    // non-symmetric tiles (split 0 only): the own block, and for an even block count the opposite block I + nb/2
-    // (a solve whose j-side rows do not fit the workspace at once is cut into bands of partner offsets d0+1 .. d0+rows;
-    // the non-symmetric tiles belong to the first band)
-    const int n_ns = (sidx == 0 && first) ? TPB * ((nb > 1 && (nb & 1) == 0) ? 2 : 1) : 0;
-    const int P = rows * TPB;                 // symmetric partner tiles of block I: blocks I+1 .. I+H (cyclic)
-    const int p0 = (int)(((int64_t)P * sidx) / S), p1 = (int)(((int64_t)P * (sidx + 1)) / S);
-    const int nt = n_ns + (p1 - p0);
+    // The tiles of block I in this band: first the non-symmetric ones (own block, and for an even block count the
+    // opposite block I + nb/2; they belong to the first band), then the symmetric partner tiles of blocks I+d0+1 ..
+    // I+d0+rows (cyclic).  The S splits cut this ONE list evenly, so the one-sided tiles do not pile up on one CTA.
+    // (A solve whose j-side rows do not fit the workspace at once is cut into bands of partner offsets.)
+    const int n_ns = first ? TPB * ((nb > 1 && (nb & 1) == 0) ? 2 : 1) : 0;
+    const int T = n_ns + rows * TPB;
+    const int g0 = (int)(((int64_t)T * sidx) / S), g1 = (int)(((int64_t)T * (sidx + 1)) / S);
+    const int nt = g1 - g0;
     auto tile_of = [&](int q) -> int {
-        if (q < n_ns) return ((q < TPB ? I : (I + nb / 2) % nb)) * TPB + q % TPB;
-        const int p = p0 + (q - n_ns);
+        const int g = g0 + q;
+        if (g < n_ns) return ((g < TPB ? I : (I + nb / 2) % nb)) * TPB + g % TPB;
+        const int p = g - n_ns;
         return ((I + 1 + d0 + p / TPB) % nb) * TPB + p % TPB;
     };
 
@@ -192,10 +195,10 @@ force_sym_f32_kernel(const float* __restrict__ packed, const float* __restrict__
         const int jbase = gt * TJ;
         mbar_wait(&full_bar[s], (uint32_t)(t / STAGES) & 1u);
         const float4* tp = reinterpret_cast<const float4*>(tiles + s * TJ * 4);
-        const bool sym = t >= n_ns;
+        const bool sym = g0 + t >= n_ns;
         const bool uni = (tm == tm) && (!sym || uni_i);
         if (!sym) {
-            const bool diag = (MODE == MODE_FORCE_POT) && !GUARD && t < TPB;   // the own block holds j == i
+            const bool diag = (MODE == MODE_FORCE_POT) && !GUARD && g0 + t < TPB;   // the own block holds j == i
             if (uni) {
                 if (diag) sweep_tile<IPT, MODE, GUARD, true, true>(tp, TJ / 2, nx, ny, nz, ax, ay, az, ap, eps2, jbase, iidx);
                 else sweep_tile<IPT, MODE, GUARD, false, true>(tp, TJ / 2, nx, ny, nz, ax, ay, az, ap, eps2, jbase, iidx);
@@ -274,7 +277,7 @@ force_sym_f32_kernel(const float* __restrict__ packed, const float* __restrict__
                 if (MODE == MODE_FORCE_POT) fp = __fadd_rn(fp, h ? e[3].y : e[3].x);
             }
             const float sj = uni ? bm : 1.0f;
-            const int row = (p0 + (t - n_ns)) / TPB;                       // d - 1
+            const int row = (g0 + t - n_ns) / TPB;                       // d - 1
             partial_j[(size_t)row * n_padb + jbase + tid] =
                 make_float4(-__fmul_rn(sj, fx), -__fmul_rn(sj, fy), -__fmul_rn(sj, fz), __fmul_rn(sj, fp));
             buf ^= 1;   // the other buffer is free: every thread passed the barrier of the tile before

@@ -7,6 +7,9 @@
 // which serves the two ordered pairs (i <- j) and (j <- i): 18 force-only (15 one-sided per ORDERED pair), 21 with the
 // potential (17), two more when the masses are not common to block and tile -- 9 / 10.5 instead of 15 / 17 per pair
 // interaction.
+#ifndef PP_SYM64_ORDER
+#define PP_SYM64_ORDER 0
+#endif
 #include "force_f64_common.cuh"
 #include <algorithm>
 
@@ -57,12 +60,21 @@ __device__ __forceinline__ void sym_chunk(double xj, double yj, double zj, doubl
             }
             const double si = UNI ? s : mj * s;               // pull of j on i:  m_j x^{-3/2} (r_j - r_i)
             const double sj = UNI ? s : mi[k] * s;            // pull of i on j: -m_i x^{-3/2} (r_j - r_i)
+#if PP_SYM64_ORDER == 1   // i-side and j-side update of one component back to back: they share two operands
+            ax[k] = fma(si, dx, ax[k]);
+            fx = fma(sj, dx, fx);
+            ay[k] = fma(si, dy, ay[k]);
+            fy = fma(sj, dy, fy);
+            az[k] = fma(si, dz, az[k]);
+            fz = fma(sj, dz, fz);
+#else
             ax[k] = fma(si, dx, ax[k]);
             ay[k] = fma(si, dy, ay[k]);
             az[k] = fma(si, dz, az[k]);
             fx = fma(sj, dx, fx);
             fy = fma(sj, dy, fy);
             fz = fma(sj, dz, fz);
+#endif
         }
         xj = rotd(xj, src); yj = rotd(yj, src); zj = rotd(zj, src);
         if (!UNI) mj = rotd(mj, src);
@@ -92,15 +104,18 @@ force_sym_f64_kernel(const double* __restrict__ packed, const double* __restrict
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int I = blockIdx.x;
     const int S = gridDim.y, sidx = blockIdx.y;
-    // (a solve whose j-side rows do not fit the workspace at once is cut into bands of partner offsets d0+1 .. d0+rows;
-    // the non-symmetric tiles belong to the first band)
-    const int n_ns = (sidx == 0 && first) ? TPB * ((nb > 1 && (nb & 1) == 0) ? 2 : 1) : 0;
-    const int P = rows * TPB;
-    const int p0 = (int)(((int64_t)P * sidx) / S), p1 = (int)(((int64_t)P * (sidx + 1)) / S);
-    const int nt = n_ns + (p1 - p0);
+    // The tiles of block I in this band: first the non-symmetric ones (own block, and for an even block count the
+    // opposite block I + nb/2; they belong to the first band), then the symmetric partner tiles of blocks I+d0+1 ..
+    // I+d0+rows (cyclic).  The S splits cut this ONE list evenly, so the one-sided tiles do not pile up on one CTA.
+    // (A solve whose j-side rows do not fit the workspace at once is cut into bands of partner offsets.)
+    const int n_ns = first ? TPB * ((nb > 1 && (nb & 1) == 0) ? 2 : 1) : 0;
+    const int T = n_ns + rows * TPB;
+    const int g0 = (int)(((int64_t)T * sidx) / S), g1 = (int)(((int64_t)T * (sidx + 1)) / S);
+    const int nt = g1 - g0;
     auto tile_of = [&](int q) -> int {
-        if (q < n_ns) return ((q < TPB ? I : (I + nb / 2) % nb)) * TPB + q % TPB;
-        const int p = p0 + (q - n_ns);
+        const int g = g0 + q;
+        if (g < n_ns) return ((g < TPB ? I : (I + nb / 2) % nb)) * TPB + g % TPB;
+        const int p = g - n_ns;
         return ((I + 1 + d0 + p / TPB) % nb) * TPB + p % TPB;
     };
 
@@ -150,10 +165,10 @@ force_sym_f64_kernel(const double* __restrict__ packed, const double* __restrict
         const int jbase = gt * TJ;
         mbar_wait(&full_bar[s], (uint32_t)(t / STAGES) & 1u);
         const double4* tp = reinterpret_cast<const double4*>(tiles + s * TJ * 4);
-        const bool sym = t >= n_ns;
+        const bool sym = g0 + t >= n_ns;
         const bool uni = (tm == tm) && (!sym || uni_i);
         if (!sym) {
-            const bool diag = (MODE == MODE_FORCE_POT) && !GUARD && t < TPB;
+            const bool diag = (MODE == MODE_FORCE_POT) && !GUARD && g0 + t < TPB;
             if (uni) {
                 if (diag) sweep_tile<IPT, MODE, GUARD, true, true>(tp, TJ, xi, yi, zi, ax, ay, az, ap, eps2, jbase, iidx);
                 else sweep_tile<IPT, MODE, GUARD, false, true>(tp, TJ, xi, yi, zi, ax, ay, az, ap, eps2, jbase, iidx);
@@ -207,7 +222,7 @@ force_sym_f64_kernel(const double* __restrict__ packed, const double* __restrict
                 if (MODE == MODE_FORCE_POT) fp += e.w;
             }
             const double sj = uni ? bm : 1.0;
-            const int row = (p0 + (t - n_ns)) / TPB;                       // d - 1
+            const int row = (g0 + t - n_ns) / TPB;                       // d - 1
             partial_j[(size_t)row * n_padb + jbase + tid] = make_double4(-(sj * fx), -(sj * fy), -(sj * fz), sj * fp);
             buf ^= 1;
         }

@@ -123,18 +123,19 @@ Plan make_sym_plan(int64_t N, int precision, int mode, int sm_count, int64_t for
     // split-j over the partner tiles of a block: fill the last wave, as make_plan does
     const int tpb = p.i_per_cta / p.tile_j;
     const int64_t ptiles = (int64_t)p.sym_h * tpb;
-    int64_t s_lo = 1, s_hi = std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(ptiles, 64),
+    int64_t s_lo = 1, s_hi = std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(ptiles + tpb, 64),
                                                                      (int64_t)((1ull << 30) / (p.part_stride * elem))));
-    if (forced_split >= 1) s_lo = s_hi = std::max<int64_t>(1, std::min<int64_t>(forced_split, std::max<int64_t>(ptiles, 1)));
+    if (forced_split >= 1) s_lo = s_hi = std::max<int64_t>(1, std::min<int64_t>(forced_split, ptiles + tpb));
     double best = -1.0;
     p.split = 1;
     for (int64_t S = s_lo; S <= s_hi; ++S) {
         const int64_t units = (int64_t)p.n_iblocks * S;
         const int64_t waves = (units + sm_count - 1) / sm_count;
-        // per unit: its share of the partner tiles + 2 tile-times of fill and epilogue; the one-sided tiles (own block,
-        // and the opposite block when the block count is even) ride on the split-0 units, i.e. once on the critical path
+        // per unit: its share of the block's tiles (the one-sided ones of the own and, for an even block count, the
+        // opposite block, plus the partner tiles) + 2 tile-times of fill and epilogue
         const double n_ns = (double)tpb * ((p.n_iblocks > 1 && p.n_iblocks % 2 == 0) ? 2.0 : 1.0);
-        const double cost = ((double)waves * ((double)((ptiles + S - 1) / S) + 2.0) + n_ns) * p.i_per_cta * p.tile_j +
+        const double per_unit = std::ceil(((double)ptiles + n_ns) / (double)S) + 2.0;
+        const double cost = (double)waves * per_unit * p.i_per_cta * p.tile_j +
                             kSymFinalizeCost * (double)S * (double)p.part_stride;
         if (best < 0.0 || cost < best * (1.0 - 1e-9)) { best = cost; p.split = (int)S; }
     }
