@@ -55,6 +55,8 @@ def parse_args():
     ap.add_argument("--no-fp64", action="store_true", help="skip the FP64 arm (faster profiling runs)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-variants", action="store_true",
+                    help="skip the unequal-mass and one-sided force-only timings (single solves at N = 2^22, 2^23)")
     ap.add_argument("--no-kdk-latency", action="store_true", help="skip the small-N step-latency rows (configs 0, 1)")
     ap.add_argument("--sweep-n", type=int, nargs=2, metavar=("LOG2_MIN", "LOG2_MAX"), default=None,
                     help="throughput of one gravity solve vs N = 2^min .. 2^max for every shape class (BASELINE.md "
@@ -248,16 +250,18 @@ def run_ours(args):
 
         fms = max_over_ranks(time_steps(torch, force_only, max(2, args.steps // 2), 1, flush, barrier))
         results[name]["force_only"] = replicas.job_value(pairs, max(2, args.steps // 2), fms, world)
-        # the same solve with m_j kept inside the pair loop on every tile (what a system of unequal masses costs)
-        ppgrav.pp_configure(ppgrav.PP_CFG_EQUAL_MASS, 0)
-        gms = max_over_ranks(time_steps(torch, force_only, 2, 1, flush, barrier))
-        ppgrav.pp_configure(ppgrav.PP_CFG_EQUAL_MASS, 1)
-        results[name]["force_only_unequal_masses"] = replicas.job_value(pairs, 2, gms, world)
-        # and with every ORDERED pair evaluated (the one-sided sweep: what N > 2^21 and i-ranges run)
-        ppgrav.pp_configure(ppgrav.PP_CFG_SYMMETRIC, 0)
-        oms = max_over_ranks(time_steps(torch, force_only, 2, 1, flush, barrier))
-        ppgrav.pp_configure(ppgrav.PP_CFG_SYMMETRIC, 1)
-        results[name]["force_only_one_sided"] = replicas.job_value(pairs, 2, oms, world)
+        results[name]["force_only_unequal_masses"] = results[name]["force_only_one_sided"] = None
+        if not args.no_variants:
+            # the same solve with m_j kept inside the pair loop on every tile (what a system of unequal masses costs)
+            ppgrav.pp_configure(ppgrav.PP_CFG_EQUAL_MASS, 0)
+            gms = max_over_ranks(time_steps(torch, force_only, 2, 1, flush, barrier))
+            ppgrav.pp_configure(ppgrav.PP_CFG_EQUAL_MASS, 1)
+            results[name]["force_only_unequal_masses"] = replicas.job_value(pairs, 2, gms, world)
+            # and with every ORDERED pair evaluated (the one-sided sweep: what i-range solves run)
+            ppgrav.pp_configure(ppgrav.PP_CFG_SYMMETRIC, 0)
+            oms = max_over_ranks(time_steps(torch, force_only, 2, 1, flush, barrier))
+            ppgrav.pp_configure(ppgrav.PP_CFG_SYMMETRIC, 1)
+            results[name]["force_only_one_sided"] = replicas.job_value(pairs, 2, oms, world)
 
         if name == "f64" and world == 1 and not args.no_kdk_latency:
             # pp_invariants with its own FP64 potential sweep (pot = NULL; what the conservation experiment pays per

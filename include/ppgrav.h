@@ -75,7 +75,7 @@ extern "C" {
 #define PP_CFG_SYMMETRIC 6 /* the pair sweep that evaluates every UNORDERED pair once (Newton's third law: one evaluation
                             * of eq. (2) serves i <- j and j <- i; 7-9 instead of 11-13 FP32-pipe operations per pair
                             * interaction, 9-11.5 instead of 15-18 FP64).  1 (default) = used for full solves (every
-                            * precision; not for i-ranges) of N >= 98304 bodies, if its j-side workspace (N^2/(2B) x 16
+                            * precision; not for i-ranges) of N >= 14000 bodies, if its j-side workspace (N^2/(2B) x 16
                             * or 32 B, B = 2048, at most 48 GB; in bands of 16 GB beyond N = 2^21) can be
                             * allocated -- otherwise the one-sided sweep runs; 0 = never; 2 = always (PP_ENOMEM if the
                             * workspace cannot be allocated) */

@@ -63,8 +63,8 @@ def test_plan_is_sane(ppgrav, prec):
                 assert p["pipe_ops_per_pair"] == ((11.5 if with_pot else 10) if prec else (9 if with_pot else 8))
             else:
                 assert p["pipe_ops_per_pair"] == ((18 if with_pot else 16) if prec else (13 if with_pot else 12))
-    # calibrated choices: one body per thread for small systems, the mid class at 2^14 (FP32),
-    # the large one-sided class at 2^15 and 2^16, the symmetric sweep from 2^17
+    # calibrated choices: one body per thread for small systems, the symmetric sweep from
+    # 2^14; with it switched off the mid class at 2^14 (FP32) and the large one-sided class from 2^15
     for n in (2 ** 17, 2 ** 20, 2 ** 23):
         p = ppgrav.pp_plan_query(n, prec)
         # full solves take the symmetric sweep; beyond 2^21 its j-side rows (> 48 GB) are worked through in bands
@@ -74,9 +74,14 @@ def test_plan_is_sane(ppgrav, prec):
         assert rows * p["i_blocks"] * p["i_per_cta"] * elem <= (16 if p["sym_bands"] > 1 else 48) << 30
     for n in (100, 1024, 2 ** 13):
         assert ppgrav.pp_plan_query(n, prec)["shape"] == 2
-    assert ppgrav.pp_plan_query(2 ** 14, prec)["shape"] == (2 if prec else 1)
-    assert ppgrav.pp_plan_query(2 ** 15, prec)["shape"] == 0 and ppgrav.pp_plan_query(2 ** 16, prec)["shape"] == 0
-    assert ppgrav.pp_plan_query(2 ** 17, prec)["shape"] == 3
+    for n in (2 ** 14, 2 ** 15, 2 ** 17):
+        assert ppgrav.pp_plan_query(n, prec)["shape"] == 3
+    ppgrav.pp_configure(ppgrav.PP_CFG_SYMMETRIC, 0)
+    try:
+        assert ppgrav.pp_plan_query(2 ** 14, prec)["shape"] == (2 if prec else 1)
+        assert ppgrav.pp_plan_query(2 ** 15, prec)["shape"] == 0 and ppgrav.pp_plan_query(2 ** 16, prec)["shape"] == 0
+    finally:
+        ppgrav.pp_configure(ppgrav.PP_CFG_SYMMETRIC, 1)
     # FP64 per-mode shapes of the large class share the tile size (so they share tile masses and padding rules)
     ppgrav.pp_configure(ppgrav.PP_CFG_SYMMETRIC, 0)
     try:
