@@ -78,7 +78,8 @@ extern "C" {
                             * precision; not for i-ranges) of N >= 14000 bodies, if its j-side workspace (N^2/(2B) x 16
                             * or 32 B, B = 2048, at most 48 GB; in bands of 16 GB beyond N = 2^21) can be
                             * allocated -- otherwise the one-sided sweep runs; 0 = never; 2 = always (PP_ENOMEM if the
-                            * workspace cannot be allocated) */
+                            * workspace cannot be allocated; PP_CFG_SHAPE = 1 / 2 then pins its 256- / 128-body j-tile
+                            * variant, which is otherwise chosen by size: 128 below N = 98304) */
 
 #define PP_CFG_SYM_BAND_ROWS 7 /* test hook: 0 (default) = the symmetric sweep keeps all its j-side rows when they fit 48 GB
                                 * and otherwise works through bands of partner offsets of at most 16 GB of rows;

@@ -289,12 +289,15 @@ bool symmetric_plan(int64_t N, int sweep_prec, int mode, int sm_count, bool full
         if (N < 14000) return false;
     }
     size_t jbytes = 0, abytes = 0;
-    Plan sp = make_sym_plan(N, sweep_prec, mode, sm_count, g_cfg_split.load(), kMaxPartialJBytes, &jbytes, &abytes);
-    if (sp.sym_bands > 1) sp = make_sym_plan(N, sweep_prec, mode, sm_count, g_cfg_split.load(), kBandBytes, &jbytes, &abytes);
+    // pinned symmetric sweep (PP_CFG_SYMMETRIC = 2): PP_CFG_SHAPE large / mid pins its 256- / 128-body tile variant
+    const int fine = cfg == 2 ? (forced_class() == CLS_LARGE ? 0 : forced_class() == CLS_MID ? 1 : -1) : -1;
+    const int64_t fs = g_cfg_split.load();
+    Plan sp = make_sym_plan(N, sweep_prec, mode, sm_count, fs, kMaxPartialJBytes, &jbytes, &abytes, fine);
+    if (sp.sym_bands > 1) sp = make_sym_plan(N, sweep_prec, mode, sm_count, fs, kBandBytes, &jbytes, &abytes, fine);
     const int64_t force_rows = g_cfg_band_rows.load();   // PP_CFG_SYM_BAND_ROWS (tests): at most that many rows per band
     if (force_rows >= 1) {
         const size_t row_bytes = (size_t)sp.part_stride * (sweep_prec == PP_F64 ? 32 : 16);
-        sp = make_sym_plan(N, sweep_prec, mode, sm_count, g_cfg_split.load(), (size_t)force_rows * row_bytes, &jbytes, &abytes);
+        sp = make_sym_plan(N, sweep_prec, mode, sm_count, fs, (size_t)force_rows * row_bytes, &jbytes, &abytes, fine);
     }
     *p = sp;
     return true;

@@ -117,7 +117,7 @@ force_sym_f32_kernel(const float* __restrict__ packed, const float* __restrict__
     constexpr int JP = kSymF32Jp;          // j-pairs a lane keeps in flight
     constexpr int CHUNKS = TJ / (64 * JP); // JP x 64 j-bodies (32 lanes x JP pairs) per systolic pass
     constexpr uint32_t TILE_BYTES = TJ * 16u;
-    static_assert(B % TJ == 0 && TJ % (64 * JP) == 0 && TJ == THREADS, "one thread per j-body in the tile reduction");
+    static_assert(B % TJ == 0 && TJ % (64 * JP) == 0 && TJ <= THREADS, "one thread per j-body in the tile reduction");
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float* tiles = reinterpret_cast<float*>(smem_raw);                                   // [STAGES][TJ*4]
     float2* jacc = reinterpret_cast<float2*>(smem_raw + STAGES * TILE_BYTES);            // [2][NWARPS][TJ/2][4]
@@ -265,7 +265,7 @@ force_sym_f32_kernel(const float* __restrict__ packed, const float* __restrict__
         // j-side: the 8 warps' sums for the TJ bodies of this tile meet here, in warp order; one thread per j-body
         if (sym) {
             __syncthreads();
-            const float2* base = jacc + ((size_t)(buf * NWARPS) * (TJ / 2)) * 4 + (size_t)(tid >> 1) * 4;
+            const float2* base = jacc + ((size_t)(buf * NWARPS) * (TJ / 2)) * 4 + (size_t)((tid < TJ ? tid : 0) >> 1) * 4;
             const int h = tid & 1;
             float fx = 0.f, fy = 0.f, fz = 0.f, fp = 0.f;
 #pragma unroll
@@ -278,8 +278,9 @@ force_sym_f32_kernel(const float* __restrict__ packed, const float* __restrict__
             }
             const float sj = uni ? bm : 1.0f;
             const int row = (g0 + t - n_ns) / TPB;                       // d - 1
-            partial_j[(size_t)row * n_padb + jbase + tid] =
-                make_float4(-__fmul_rn(sj, fx), -__fmul_rn(sj, fy), -__fmul_rn(sj, fz), __fmul_rn(sj, fp));
+            if (tid < TJ)
+                partial_j[(size_t)row * n_padb + jbase + tid] =
+                    make_float4(-__fmul_rn(sj, fx), -__fmul_rn(sj, fy), -__fmul_rn(sj, fz), __fmul_rn(sj, fp));
             buf ^= 1;   // the other buffer is free: every thread passed the barrier of the tile before
         }
     }
@@ -295,10 +296,10 @@ force_sym_f32_kernel(const float* __restrict__ packed, const float* __restrict__
     }
 }
 
-template <int MODE, bool GUARD>
+template <int FINE, int MODE, bool GUARD>
 int launch_mg(const Plan& p, const float* packed, const float* tile_mass, const float* block_mass, float4* partial,
               float4* partial_j, float4* acc_j, float eps2, cudaStream_t st) {
-    constexpr KernelShape K = kShapeF32Sym;
+    constexpr KernelShape K = FINE ? kShapeF32SymFine : kShapeF32Sym;
     // j-tile ring + two j-side reduction buffers + mbarriers + the outer sums
     constexpr size_t smem = (size_t)K.stages * K.tile_j * 16 + 2 * (K.threads / 32) * (K.tile_j / 2) * 32 + 2 * K.stages * 8 +
                             (size_t)8 * K.ipt * K.threads * 4;
@@ -319,22 +320,31 @@ int launch_mg(const Plan& p, const float* packed, const float* tile_mass, const 
     return PP_OK;
 }
 
+template <int FINE>
+int launch_fine(const Plan& p, const float* packed, const float* tile_mass, const float* block_mass, float4* partial,
+                float4* partial_j, float4* acc_j, float eps2, bool guard, int mode, cudaStream_t st) {
+    if (mode == MODE_FORCE)
+        return guard ? launch_mg<FINE, MODE_FORCE, true>(p, packed, tile_mass, block_mass, partial, partial_j, acc_j, eps2, st)
+                     : launch_mg<FINE, MODE_FORCE, false>(p, packed, tile_mass, block_mass, partial, partial_j, acc_j, eps2, st);
+    return guard ? launch_mg<FINE, MODE_FORCE_POT, true>(p, packed, tile_mass, block_mass, partial, partial_j, acc_j, eps2, st)
+                 : launch_mg<FINE, MODE_FORCE_POT, false>(p, packed, tile_mass, block_mass, partial, partial_j, acc_j, eps2, st);
+}
+
 }  // namespace
 
 int launch_force_sym_f32(const Plan& p, const float* packed, const float* tile_mass, const float* block_mass,
                          float4* partial, float4* partial_j, float4* acc_j, double delta, int mode, cudaStream_t st) {
-    constexpr KernelShape K = kShapeF32Sym;
-    if (!p.sym || p.threads != K.threads || p.ipt != K.ipt || p.tile_j != K.tile_j || p.i_begin != 0) {
+    constexpr KernelShape K = kShapeF32Sym, F = kShapeF32SymFine;
+    const bool fine = p.tile_j == F.tile_j;
+    if (!p.sym || p.threads != K.threads || p.ipt != K.ipt || (p.tile_j != K.tile_j && !fine) || p.i_begin != 0 ||
+        (mode != MODE_FORCE && mode != MODE_FORCE_POT)) {
         set_error("launch_force_sym_f32: not a symmetric FP32 plan");
         return PP_EINVAL;
     }
     const float eps2 = (float)(delta * delta);
     const bool guard = !(eps2 >= kTinyR2F32);
-    if (mode == MODE_FORCE)
-        return guard ? launch_mg<MODE_FORCE, true>(p, packed, tile_mass, block_mass, partial, partial_j, acc_j, eps2, st)
-                     : launch_mg<MODE_FORCE, false>(p, packed, tile_mass, block_mass, partial, partial_j, acc_j, eps2, st);
-    return guard ? launch_mg<MODE_FORCE_POT, true>(p, packed, tile_mass, block_mass, partial, partial_j, acc_j, eps2, st)
-                 : launch_mg<MODE_FORCE_POT, false>(p, packed, tile_mass, block_mass, partial, partial_j, acc_j, eps2, st);
+    return fine ? launch_fine<1>(p, packed, tile_mass, block_mass, partial, partial_j, acc_j, eps2, guard, mode, st)
+                : launch_fine<0>(p, packed, tile_mass, block_mass, partial, partial_j, acc_j, eps2, guard, mode, st);
 }
 
 }  // namespace ppgrav

@@ -94,7 +94,7 @@ force_sym_f64_kernel(const double* __restrict__ packed, const double* __restrict
     constexpr int TPB = B / TJ;
     constexpr int CHUNKS = TJ / 32;
     constexpr uint32_t TILE_BYTES = TJ * 32u;
-    static_assert(B % TJ == 0 && TJ % 32 == 0 && TJ == THREADS, "one thread per j-body in the tile reduction");
+    static_assert(B % TJ == 0 && TJ % 32 == 0 && TJ <= THREADS, "one thread per j-body in the tile reduction");
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double* tiles = reinterpret_cast<double*>(smem_raw);                                  // [STAGES][TJ*4]
     double4* jacc = reinterpret_cast<double4*>(smem_raw + STAGES * TILE_BYTES);           // [2][NWARPS][TJ]
@@ -213,7 +213,7 @@ force_sym_f64_kernel(const double* __restrict__ packed, const double* __restrict
 
         if (sym) {   // j-side: the 8 warps' sums for the TJ bodies of this tile, added in warp order, one thread per body
             __syncthreads();
-            const double4* base = jacc + (size_t)(buf * NWARPS) * TJ + tid;
+            const double4* base = jacc + (size_t)(buf * NWARPS) * TJ + (tid < TJ ? tid : 0);
             double fx = 0.0, fy = 0.0, fz = 0.0, fp = 0.0;
 #pragma unroll
             for (int w = 0; w < NWARPS; ++w) {
@@ -223,7 +223,8 @@ force_sym_f64_kernel(const double* __restrict__ packed, const double* __restrict
             }
             const double sj = uni ? bm : 1.0;
             const int row = (g0 + t - n_ns) / TPB;                       // d - 1
-            partial_j[(size_t)row * n_padb + jbase + tid] = make_double4(-(sj * fx), -(sj * fy), -(sj * fz), sj * fp);
+            if (tid < TJ)
+                partial_j[(size_t)row * n_padb + jbase + tid] = make_double4(-(sj * fx), -(sj * fy), -(sj * fz), sj * fp);
             buf ^= 1;
         }
     }
@@ -234,10 +235,10 @@ force_sym_f64_kernel(const double* __restrict__ packed, const double* __restrict
             make_double4(os(0, k), os(1, k), os(2, k), (MODE == MODE_FORCE_POT) ? os(3, k) : 0.0);
 }
 
-template <int MODE, bool GUARD>
+template <int FINE, int MODE, bool GUARD>
 int launch_mg(const Plan& p, const double* packed, const double* tile_mass, const double* block_mass, double4* partial,
               double4* partial_j, double4* acc_j, double eps2, cudaStream_t st) {
-    constexpr KernelShape K = kShapeF64Sym;
+    constexpr KernelShape K = FINE ? kShapeF64SymFine : kShapeF64Sym;
     // j-tile ring + two j-side reduction buffers + mbarriers + the outer sums
     constexpr size_t smem = (size_t)K.stages * K.tile_j * 32 + 2 * (K.threads / 32) * K.tile_j * 32 + 2 * K.stages * 8 +
                             (size_t)4 * K.ipt * K.threads * 8;
@@ -259,25 +260,31 @@ int launch_mg(const Plan& p, const double* packed, const double* tile_mass, cons
     return PP_OK;
 }
 
+template <int FINE>
+int launch_fine(const Plan& p, const double* packed, const double* tile_mass, const double* block_mass, double4* partial,
+                double4* partial_j, double4* acc_j, double eps2, bool guard, int mode, cudaStream_t st) {
+    if (mode == MODE_FORCE)
+        return guard ? launch_mg<FINE, MODE_FORCE, true>(p, packed, tile_mass, block_mass, partial, partial_j, acc_j, eps2, st)
+                     : launch_mg<FINE, MODE_FORCE, false>(p, packed, tile_mass, block_mass, partial, partial_j, acc_j, eps2, st);
+    return guard ? launch_mg<FINE, MODE_FORCE_POT, true>(p, packed, tile_mass, block_mass, partial, partial_j, acc_j, eps2, st)
+                 : launch_mg<FINE, MODE_FORCE_POT, false>(p, packed, tile_mass, block_mass, partial, partial_j, acc_j, eps2, st);
+}
+
 }  // namespace
 
 int launch_force_sym_f64(const Plan& p, const double* packed, const double* tile_mass, const double* block_mass,
                          double4* partial, double4* partial_j, double4* acc_j, double delta, int mode, cudaStream_t st) {
-    constexpr KernelShape K = kShapeF64Sym;
-    if (!p.sym || p.threads != K.threads || p.ipt != K.ipt || p.tile_j != K.tile_j || p.i_begin != 0) {
+    constexpr KernelShape K = kShapeF64Sym, F = kShapeF64SymFine;
+    const bool fine = p.tile_j == F.tile_j;
+    if (!p.sym || p.threads != K.threads || p.ipt != K.ipt || (p.tile_j != K.tile_j && !fine) || p.i_begin != 0 ||
+        (mode != MODE_FORCE && mode != MODE_FORCE_POT)) {
         set_error("launch_force_sym_f64: not a symmetric FP64 plan");
         return PP_EINVAL;
     }
     const double eps2 = delta * delta;
     const bool guard = !(eps2 >= kTinyR2F64);
-    if (mode == MODE_FORCE)
-        return guard ? launch_mg<MODE_FORCE, true>(p, packed, tile_mass, block_mass, partial, partial_j, acc_j, eps2, st)
-                     : launch_mg<MODE_FORCE, false>(p, packed, tile_mass, block_mass, partial, partial_j, acc_j, eps2, st);
-    if (mode == MODE_FORCE_POT)
-        return guard ? launch_mg<MODE_FORCE_POT, true>(p, packed, tile_mass, block_mass, partial, partial_j, acc_j, eps2, st)
-                     : launch_mg<MODE_FORCE_POT, false>(p, packed, tile_mass, block_mass, partial, partial_j, acc_j, eps2, st);
-    set_error("launch_force_sym_f64: mode %d has no symmetric kernel", mode);
-    return PP_EINVAL;
+    return fine ? launch_fine<1>(p, packed, tile_mass, block_mass, partial, partial_j, acc_j, eps2, guard, mode, st)
+                : launch_fine<0>(p, packed, tile_mass, block_mass, partial, partial_j, acc_j, eps2, guard, mode, st);
 }
 
 }  // namespace ppgrav

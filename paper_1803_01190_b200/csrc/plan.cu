@@ -99,8 +99,10 @@ Plan make_plan(int64_t N, int precision, int mode, int sm_count, int64_t forced_
 }
 
 Plan make_sym_plan(int64_t N, int precision, int mode, int sm_count, int64_t forced_split, size_t rows_cap_bytes,
-                   size_t* jbytes, size_t* abytes) {
-    const KernelShape& d = precision == PP_F64 ? kShapeF64Sym : kShapeF32Sym;
+                   size_t* jbytes, size_t* abytes, int fine_tiles) {
+    const bool fine = fine_tiles < 0 ? N < kSymFineBelow : fine_tiles != 0;
+    const KernelShape& d = precision == PP_F64 ? (fine ? kShapeF64SymFine : kShapeF64Sym)
+                                               : (fine ? kShapeF32SymFine : kShapeF32Sym);
     const size_t elem = precision == PP_F64 ? 32 : 16;
     Plan p{};
     p.cls = CLS_LARGE;

@@ -128,6 +128,11 @@ constexpr int kSymF32Unroll = PP_SYM32_UNROLL;  // systolic steps per unrolled l
 constexpr int kSymF64Unroll = PP_SYM64_UNROLL;
 constexpr KernelShape kShapeF32Sym = {256, PP_SYM32_IPT, 256, 4, 1};
 constexpr KernelShape kShapeF64Sym = {256, PP_SYM64_IPT, 256, 4, 1};
+// the same kernels on 128-body tiles: half the work unit, for the sizes (N < 2^17) where a solve is only 1-2 waves of
+// CTAs and the granularity of a 29-us tile costs more than the doubled per-tile overhead
+constexpr KernelShape kShapeF32SymFine = {256, PP_SYM32_IPT, 128, 4, 1};
+constexpr KernelShape kShapeF64SymFine = {256, PP_SYM64_IPT, 128, 4, 1};
+constexpr int64_t kSymFineBelow = 98304;
 constexpr KernelShape kShapes[2][kNumClasses][kNumModes] = {
     {{kShapeF32Large, kShapeF32Large, kShapeF32Large},
      {kShapeF32Mid, kShapeF32Mid, kShapeF32Mid},
@@ -172,8 +177,9 @@ Plan make_plan(int64_t N, int precision, int mode, int sm_count, int64_t forced_
 // plan of the symmetric sweep for a full solve of N bodies; bytes of its j-side workspace in *jbytes
 // (rows_cap_bytes: the j-side rows of one band may take that much; *jbytes = bytes of partial_j, *abytes = bytes of
 // the running j-side sums acc_j that bands need, 0 for a single band)
+// fine_tiles: 1 = 128-body j-tiles, 0 = 256-body, -1 = by size (128 below kSymFineBelow)
 Plan make_sym_plan(int64_t N, int precision, int mode, int sm_count, int64_t forced_split, size_t rows_cap_bytes,
-                   size_t* jbytes, size_t* abytes);
+                   size_t* jbytes, size_t* abytes, int fine_tiles = -1);
 
 // ---- kernels (one launcher per translation unit) -----------------------------------------------------------------
 // Packed bodies.  FP32: pairs of bodies interleaved, 8 floats {x0 x1 y0 y1 z0 z1 m0 m1} per pair (so that one

@@ -58,7 +58,7 @@ def test_plan_is_sane(ppgrav, prec):
             elem = 32 if prec else 16
             assert p["split"] * n_ib * p["i_per_cta"] * elem <= (1 << 30) or p["split"] == 1
             if p["shape"] == 3:                    # symmetric sweep: one evaluation serves two ordered pairs
-                assert (p["i_per_cta"], p["tile_j"]) == (2048, 256)
+                assert (p["i_per_cta"], p["tile_j"]) == (2048, 128 if n < 98304 else 256)
                 assert p["pairs_per_evaluation"] == 2 and p["sym_partner_blocks"] == (n_ib - 1) // 2
                 assert p["pipe_ops_per_pair"] == ((11.5 if with_pot else 10) if prec else (9 if with_pot else 8))
             else:

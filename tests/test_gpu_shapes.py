@@ -366,19 +366,22 @@ def test_two_streams_share_the_workspace_safely(gpu):
 
 # ---- the symmetric sweep (every unordered pair once, force_sym_f32.cu) ---------------------------------------------
 class _Symmetric:
-    """PP_CFG_SYMMETRIC = 2 (always) for the duration of a with-block, optionally with a pinned split-j."""
+    """PP_CFG_SYMMETRIC = 2 (always) for the duration of a with-block, optionally with a pinned split-j and a pinned
+    j-tile variant (256: what N >= 98304 runs, i.e. the bench; 128: what smaller systems run; 0: by size)."""
 
-    def __init__(self, gpu, split=0):
-        self.gpu, self.split = gpu, split
+    def __init__(self, gpu, split=0, tile=0):
+        self.gpu, self.split, self.tile = gpu, split, tile
 
     def __enter__(self):
         self.gpu.pp_configure(self.gpu.PP_CFG_SYMMETRIC, 2)
         self.gpu.pp_configure(self.gpu.PP_CFG_SPLIT_J, self.split)
+        self.gpu.pp_configure(self.gpu.PP_CFG_SHAPE, {0: 0, 256: 1, 128: 2}[self.tile])
         return self
 
     def __exit__(self, *exc):
         self.gpu.pp_configure(self.gpu.PP_CFG_SYMMETRIC, 1)
         self.gpu.pp_configure(self.gpu.PP_CFG_SPLIT_J, 0)
+        self.gpu.pp_configure(self.gpu.PP_CFG_SHAPE, 0)
 
 
 # one block; two blocks (even: no symmetric partner, the opposite block one-sided); three (odd, H = 1); four (H = 1 and
@@ -388,8 +391,9 @@ SYM_N = [1, 2, 255, 2047, 2049, 4097, 6145, 8193, 10241, 12289, 15000, 18433]
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32", "mixed"])
+@pytest.mark.parametrize("tile", [256, 128])
 @pytest.mark.parametrize("n", SYM_N)
-def test_symmetric_sweep_edge_sizes(gpu, oracle, prec, n):
+def test_symmetric_sweep_edge_sizes(gpu, oracle, prec, tile, n):
     """All bodies against the oracle, split-j {auto, 1, 3}, random masses and mass species, with and without potential."""
     seen = "f64" if prec == "f64" else "f32"
     for masses in ("random", "species"):
@@ -398,9 +402,9 @@ def test_symmetric_sweep_edge_sizes(gpu, oracle, prec, n):
         a_ref, p_ref = _oracle_forces(oracle, (n, "sym" + seen, masses), ps, ms, 2.5, 0.05)
         dpos, dmass = _dev("f32" if prec == "f32" else "f64", ps if prec != "mixed" else pos, ms if prec != "mixed" else mass)
         for split in (0, 1, 3):
-            with _Symmetric(gpu, split):
+            with _Symmetric(gpu, split, tile):
                 plan = gpu.pp_plan_query(n, gpu.PP_F64 if prec == "f64" else gpu.PP_F32, True)
-                assert plan["shape"] == 3 and plan["i_per_cta"] == 2048 and plan["tile_j"] == 256
+                assert plan["shape"] == 3 and plan["i_per_cta"] == 2048 and plan["tile_j"] == tile
                 acc, pot = gpu.pp_forces(dpos, dmass, G=2.5, delta=0.05, want_pot=True, mixed=(prec == "mixed"))
                 acc2, _ = gpu.pp_forces(dpos, dmass, G=2.5, delta=0.05, want_pot=False, mixed=(prec == "mixed"))
             if n == 1:
@@ -412,8 +416,9 @@ def test_symmetric_sweep_edge_sizes(gpu, oracle, prec, n):
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("tile", [256, 128])
 @pytest.mark.parametrize("masses", ["random", "species"])
-def test_symmetric_sweep_delta_zero_and_bitwise_reproducible(gpu, oracle, prec, masses):
+def test_symmetric_sweep_delta_zero_and_bitwise_reproducible(gpu, oracle, prec, tile, masses):
     import torch
     n = 9001
     pos, _, mass = _cloud(n, 93, masses)
@@ -421,7 +426,7 @@ def test_symmetric_sweep_delta_zero_and_bitwise_reproducible(gpu, oracle, prec, 
     a, b = 7, 6000                       # a coincident pair in two different 2048-body blocks: met in a symmetric tile
     pos[b] = pos[a]
     dpos, dmass = _dev(prec, pos, mass)
-    with _Symmetric(gpu):
+    with _Symmetric(gpu, 0, tile):
         acc, pot = gpu.pp_forces(dpos, dmass, delta=0.0, want_pot=True)
         acc_b, pot_b = gpu.pp_forces(dpos, dmass, delta=0.0, want_pot=True)
     assert torch.equal(acc, acc_b) and torch.equal(pot, pot_b)
@@ -460,7 +465,7 @@ def test_symmetric_sweep_in_bands(gpu, oracle, prec, band_rows):
     gpu.pp_configure(gpu.PP_CFG_SYM_BAND_ROWS, band_rows)
     try:
         for split in (1, 3):
-            with _Symmetric(gpu, split):
+            with _Symmetric(gpu, split, 256 if split == 1 else 128):
                 plan = gpu.pp_plan_query(n, gpu.PP_F64 if prec == "f64" else gpu.PP_F32, True)
                 assert plan["shape"] == 3 and plan["sym_bands"] == -(-plan["sym_partner_blocks"] // band_rows) >= 2
                 acc, pot = gpu.pp_forces(dpos, dmass, G=2.5, delta=0.05, want_pot=True, mixed=mixed)
@@ -518,7 +523,7 @@ def test_symmetric_sweep_trajectory_at_2p15(gpu, oracle, prec):
     dpos, dvel, dmass = _dev(prec, pos, vel, mass)
     dacc = torch.zeros_like(dpos)
     dpot = torch.empty_like(dmass)
-    with _Symmetric(gpu):
+    with _Symmetric(gpu, 0, 256):      # the tile variant of the bench kernels (the plan would take 128-body tiles here)
         gpu.pp_step_kdk(dpos, dvel, dmass, dacc, c["dt"], 5, G=c["G"], delta=c["delta"], pot=dpot)
     assert np.abs(dpos.cpu().numpy() - p_ref).max() / np.abs(p_ref).max() <= TOL_TRAJ[prec]
     assert np.abs(dvel.cpu().numpy() - v_ref).max() / np.abs(v_ref).max() <= TOL_TRAJ[prec]
