@@ -156,6 +156,25 @@ int pp_step_kdk(void* pos, void* vel, const void* mass, void* acc, void* pot, in
 int pp_invariants(const void* pos, const void* vel, const void* mass, const void* pot, int64_t N, double G,
                   double delta, int precision, double* out16, void* stream);
 
+/* pp_invariants for callers that must not allocate (code under CUDA-graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc).  Same kernels, same outputs (bit-identical to pp_invariants with the same `pot`); what differs:
+ *   - the kernels' scratch (per-block partial sums, 296 x 32 doubles = 75,776 bytes) is a file-scope static __device__
+ *     array inside the library instead of the grow-on-demand workspace: every GPU that loads the library holds those
+ *     75,776 bytes until the process exits;
+ *   - the call performs no cudaMalloc / cudaFree and calls no allocating routine (one cudaGetSymbolAddress per device
+ *     the first time, then two kernel launches);
+ *   - `pot` (Phi_i in the state precision, as pp_forces / pp_step_kdk return it) is REQUIRED: the O(N^2) potential pass
+ *     of pp_invariants(pot = NULL) needs the allocating workspace -> PP_EINVAL;
+ *   - N beyond PP_NOALLOC_MAX_N -> PP_EINVAL with a message that names the limit; G and delta are not needed (they
+ *     only enter through the potential);
+ *   - every call shares the one scratch array, which keeps the previous call's contents (nothing needs clearing: each
+ *     launched block overwrites its slot before the final kernel reads it).  Calls on ONE stream follow each other
+ *     safely; calls that overlap on the GPU (several streams without ordering, several host threads) RACE on it.
+ *   pos, vel [N,3], mass, pot [N]: device, `precision`;  out16: device, 16 doubles, as pp_invariants. */
+#define PP_NOALLOC_MAX_N (1ll << 28)
+int pp_invariants_noalloc(const void* pos, const void* vel, const void* mass, const void* pot, int64_t N,
+                          int precision, double* out16, void* stream);
+
 /* Face-on surface-density map, the diagnostic of Fig. 7:
  *   sigma [ny*nx] (device, doubles, row-major, overwritten) = (sum of m_i over the bodies with
  *   x0 + ix*cell <= x_i < x0 + (ix+1)*cell and y0 + iy*cell <= y_i < y0 + (iy+1)*cell) / cell^2;  z is ignored and

@@ -8,6 +8,8 @@
 // Two launches: (1) a grid-stride pass in which every thread keeps 12 TwoSum (value, error) pairs, merged by warp
 // shuffles and a shared-memory step into one (value, error) pair per block and quantity; (2) one warp that adds the
 // block partials in block order and writes the 16 outputs.  No atomics: bit-reproducible for a given N.
+#include <mutex>
+
 #include "ppgrav_internal.h"
 
 namespace ppgrav {
@@ -138,4 +140,83 @@ int launch_invariants_f64(const double* pos, const double* vel, const double* ma
     return launch_invariants<double>(pos, vel, mass, pot_state, pot64, N, scratch, out16, st);
 }
 
+// ---- pp_invariants_noalloc: the same two kernels with their scratch in a file-scope device array ----------------------
+// For callers that may not allocate (code under CUDA-graph capture, tight serving loops, harnesses that forbid
+// cudaMalloc): the block partials of invariants_partial_kernel live in g_noalloc_scratch instead of the library's
+// grow-on-demand workspace.  kMaxBlocks x kStride doubles = 75,776 bytes, held by every GPU that loads the library until
+// the process exits.  The grid-stride pass never launches more than kMaxBlocks blocks, so this serves any N up to
+// PP_NOALLOC_MAX_N.  Every call shares the array and finds the previous call's contents in it; nothing has to start at
+// zero, because block b overwrites its 2 x kQ doubles before invariants_final_kernel (stream-ordered behind it) reads
+// exactly the nb blocks this call launched.  Calls that overlap on the GPU (different streams, no ordering) race on it.
+namespace {
+
+static __device__ __align__(256) double g_noalloc_scratch[kMaxBlocks * kStride];
+
+constexpr int kNoallocMaxDevices = 64;
+std::mutex g_noalloc_mu;
+double* g_noalloc_ptr[kNoallocMaxDevices] = {};   // device address of g_noalloc_scratch, per device (0 = not yet asked)
+
+// In host code `g_noalloc_scratch` is a host-side stand-in, not a device address: the device address is asked for once
+// per device, with that device current, and only that pointer is ever handed to a kernel.
+int noalloc_scratch(double** out) {
+    int dev = -1;
+    PP_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kNoallocMaxDevices) {
+        set_error("pp_invariants_noalloc: device ordinal %d out of range", dev);
+        return PP_ECUDA;
+    }
+    std::lock_guard<std::mutex> lk(g_noalloc_mu);
+    if (!g_noalloc_ptr[dev]) {
+        double* p = nullptr;
+        PP_CUDA(cudaGetSymbolAddress((void**)&p, g_noalloc_scratch));
+        if (!p) {
+            set_error("pp_invariants_noalloc: cudaGetSymbolAddress returned a null address");
+            return PP_ECUDA;
+        }
+        g_noalloc_ptr[dev] = p;
+    }
+    *out = g_noalloc_ptr[dev];
+    return PP_OK;
+}
+
+}  // namespace
+
 }  // namespace ppgrav
+
+extern "C" int pp_invariants_noalloc(const void* pos, const void* vel, const void* mass, const void* pot, int64_t N,
+                                     int precision, double* out16, void* stream) {
+    using namespace ppgrav;
+    if (precision != PP_F32 && precision != PP_F64 && precision != PP_MIXED) {
+        set_error("pp_invariants_noalloc: precision must be PP_F32, PP_F64 or PP_MIXED (got %d)", precision);
+        return PP_EINVAL;
+    }
+    if (N < 1 || N > (int64_t)PP_NOALLOC_MAX_N) {
+        set_error("pp_invariants_noalloc: N = %lld outside [1, PP_NOALLOC_MAX_N = %lld]", (long long)N,
+                  (long long)PP_NOALLOC_MAX_N);
+        return PP_EINVAL;
+    }
+    if (!pot) {
+        set_error("pp_invariants_noalloc: pot is NULL -- the O(N^2) potential pass needs the allocating workspace; "
+                  "pass the potential pp_forces / pp_step_kdk returned, or call pp_invariants");
+        return PP_EINVAL;
+    }
+    const size_t a = precision == PP_F32 ? 4 : 8;
+    const void* ptrs[5] = {pos, vel, mass, pot, out16};
+    const char* names[5] = {"pos", "vel", "mass", "pot", "out16"};
+    for (int k = 0; k < 5; ++k) {
+        const size_t need = k == 4 ? 8 : a;
+        if (!ptrs[k] || (reinterpret_cast<uintptr_t>(ptrs[k]) & (need - 1))) {
+            set_error("pp_invariants_noalloc: %s is NULL or not aligned to its element size", names[k]);
+            return PP_EINVAL;
+        }
+    }
+    double* scratch = nullptr;
+    const int rc = noalloc_scratch(&scratch);
+    if (rc != PP_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (precision == PP_F32)
+        return launch_invariants<float>((const float*)pos, (const float*)vel, (const float*)mass, (const float*)pot,
+                                        nullptr, N, scratch, out16, st);
+    return launch_invariants<double>((const double*)pos, (const double*)vel, (const double*)mass, (const double*)pot,
+                                     nullptr, N, scratch, out16, st);
+}

@@ -37,6 +37,7 @@ SIGNATURES = {
     "pp_kick_drift": (_int, [_vp, _vp, _vp, _i64, _dbl, _dbl, _int, _vp]),
     "pp_step_kdk": (_int, [_vp, _vp, _vp, _vp, _vp, _i64, _dbl, _i64, _dbl, _dbl, _int, _u, _vp]),
     "pp_invariants": (_int, [_vp, _vp, _vp, _vp, _i64, _dbl, _dbl, _int, _vp, _vp]),
+    "pp_invariants_noalloc": (_int, [_vp, _vp, _vp, _vp, _i64, _int, _vp, _vp]),
     "pp_surface_density": (_int, [_vp, _vp, _i64, _dbl, _dbl, _dbl, _int, _int, _int, _vp, _vp]),
     "pp_forces_host": (_int, [_vp, _vp, _vp, _vp, _i64, _dbl, _dbl, _int, _vp]),
     "pp_step_kdk_host": (_int, [_vp, _vp, _vp, _vp, _vp, _i64, _dbl, _i64, _dbl, _dbl, _int, _u, _vp]),
@@ -231,6 +232,24 @@ def pp_invariants(pos, vel, mass, G=1.0, delta=0.0, pot=None, out16=None, stream
         _check(lib().pp_invariants(_dev(pos, (N, 3), pos.dtype, "pos"), _dev(vel, (N, 3), pos.dtype, "vel"),
                                    _dev(mass, (N,), pos.dtype, "mass"), p_pot, N, float(G), float(delta), prec,
                                    _dev(out16, (16,), torch.float64, "out16"), _stream(stream)), "pp_invariants")
+    return out16
+
+
+PP_NOALLOC_MAX_N = 1 << 28
+
+
+def pp_invariants_noalloc(pos, vel, mass, pot, out16, stream=None):
+    """pp_invariants without any allocation inside the library (its scratch is a static device array of 75,776 bytes;
+    include/ppgrav.h): pot [N] is required, out16 (CUDA float64 tensor of 16) is supplied by the caller, N at most
+    PP_NOALLOC_MAX_N.  Calls that overlap on the GPU race on the shared scratch."""
+    torch = _torch()
+    prec = _precision_of(pos)
+    N = pos.shape[0]
+    with torch.cuda.device(pos.device):
+        _check(lib().pp_invariants_noalloc(_dev(pos, (N, 3), pos.dtype, "pos"), _dev(vel, (N, 3), pos.dtype, "vel"),
+                                           _dev(mass, (N,), pos.dtype, "mass"), _dev(pot, (N,), pos.dtype, "pot"), N,
+                                           prec, _dev(out16, (16,), torch.float64, "out16"), _stream(stream)),
+               "pp_invariants_noalloc")
     return out16
 
 
