@@ -40,7 +40,7 @@ FP32_LANES, FP64_LANES, SM_COUNT, SM_MAX_HZ = 128, 64, 148, 1.965e9
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE sweep launch (with potential) at N = 2^20, from the
 # `ncu --set full` captures summarised in profiles/r2_force_sym_f32_ncu.md / profiles/r2_force_sym_f64_ncu.md (the
 # symmetric sweeps: the writes are their j-side rows, N^2/(2 x 2048) x 16 or 32 B, written once)
-NCU_TRAFFIC_BYTES = {("f32", 1 << 20): 136.68864e6 + 4267.070e6, ("f64", 1 << 20): 381.68704e6 + 8597.523e6}
+NCU_TRAFFIC_BYTES = {("f32", 1 << 20): 159.560448e6 + 4267.639e6, ("f64", 1 << 20): 406.194688e6 + 8599.203e6}
 L2_FLUSH_BYTES = 256 << 20
 
 
