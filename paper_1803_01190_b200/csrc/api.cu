@@ -14,11 +14,19 @@
 #include <utility>
 #include <vector>
 
+#include <nvtx3/nvToolsExt.h>
+
 #include "ppgrav_internal.h"
 
 namespace ppgrav {
 
 namespace {
+
+// NVTX range around an ABI call (header-only nvtx3: a no-op unless a profiler is attached)
+struct NvtxRange {
+    explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+    ~NvtxRange() { nvtxRangePop(); }
+};
 
 thread_local char t_err[512] = "";
 std::atomic<int64_t> g_launches{0};
@@ -546,6 +554,7 @@ int pp_equal_mass_tiles(const void* mass, int64_t N, int precision, int64_t* out
 
 int pp_forces_range(const void* pos, const void* mass, void* acc, void* pot, int64_t N, int64_t i_begin,
                     int64_t i_count, double G, double delta, int precision, void* stream) {
+    NvtxRange nvtx_range("pp_forces_range");
     PP_TRY(check_common("pp_forces_range", N, G, delta, precision));
     PP_TRY(check_ptr("pp_forces_range", "pos", pos, precision, true));
     PP_TRY(check_ptr("pp_forces_range", "mass", mass, precision, true));
@@ -593,6 +602,7 @@ int pp_kick_drift(void* pos, void* vel, const void* acc, int64_t n, double kick,
 
 int pp_step_kdk(void* pos, void* vel, const void* mass, void* acc, void* pot, int64_t N, double dt, int64_t nsteps,
                 double G, double delta, int precision, unsigned flags, void* stream) {
+    NvtxRange nvtx_range("pp_step_kdk");
     PP_TRY(check_common("pp_step_kdk", N, G, delta, precision));
     PP_TRY(check_ptr("pp_step_kdk", "pos", pos, precision, true));
     PP_TRY(check_ptr("pp_step_kdk", "vel", vel, precision, true));
@@ -723,6 +733,7 @@ int pp_surface_density(const void* pos, const void* mass, int64_t N, double x0, 
 
 int pp_invariants(const void* pos, const void* vel, const void* mass, const void* pot, int64_t N, double G,
                   double delta, int precision, double* out16, void* stream) {
+    NvtxRange nvtx_range("pp_invariants");
     PP_TRY(check_common("pp_invariants", N, G, delta, precision));
     PP_TRY(check_ptr("pp_invariants", "pos", pos, precision, true));
     PP_TRY(check_ptr("pp_invariants", "vel", vel, precision, true));
