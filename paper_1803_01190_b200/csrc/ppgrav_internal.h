@@ -108,6 +108,9 @@ constexpr KernelShape kShapeF64Mid = {PP_F64_MID_THREADS, PP_F64_MID_IPT, PP_F64
 constexpr KernelShape kShapeF64Small = {128, 1, 128, 4, 4};
 // shape of the symmetric (every unordered pair once) sweeps: the block must be a whole number of tiles and a tile has
 // one body per thread (its j-side sums are reduced one thread per body)
+#ifndef PP_SYM32_THREADS
+#define PP_SYM32_THREADS 256
+#endif
 #ifndef PP_SYM32_IPT
 #define PP_SYM32_IPT 8
 #endif
@@ -126,11 +129,11 @@ constexpr KernelShape kShapeF64Small = {128, 1, 128, 4, 4};
 constexpr int kSymF32Jp = PP_SYM32_JP;          // j-pairs a lane keeps in flight (force_sym_f32.cu)
 constexpr int kSymF32Unroll = PP_SYM32_UNROLL;  // systolic steps per unrolled loop body
 constexpr int kSymF64Unroll = PP_SYM64_UNROLL;
-constexpr KernelShape kShapeF32Sym = {256, PP_SYM32_IPT, 256, 4, 1};
+constexpr KernelShape kShapeF32Sym = {PP_SYM32_THREADS, PP_SYM32_IPT, 256, 4, 1};
 constexpr KernelShape kShapeF64Sym = {256, PP_SYM64_IPT, 256, 4, 1};
 // the same kernels on 128-body tiles: half the work unit, for the sizes (N < 2^17) where a solve is only 1-2 waves of
 // CTAs and the granularity of a 29-us tile costs more than the doubled per-tile overhead
-constexpr KernelShape kShapeF32SymFine = {256, PP_SYM32_IPT, 128, 4, 1};
+constexpr KernelShape kShapeF32SymFine = {PP_SYM32_THREADS, PP_SYM32_IPT, 128, 4, 1};
 constexpr KernelShape kShapeF64SymFine = {256, PP_SYM64_IPT, 128, 4, 1};
 constexpr int64_t kSymFineBelow = 98304;
 constexpr KernelShape kShapes[2][kNumClasses][kNumModes] = {
