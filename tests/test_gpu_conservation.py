@@ -43,3 +43,18 @@ def test_checkpointed_run_continues_bit_for_bit(tmp_path):
     second = conservation.run(10, 40, 5e-4, 10, "f32", verbose=False, checkpoint=ck)
     assert second["steps"] == 40 and second["times"] == whole["times"]
     assert second["E"] == whole["E"] and second["P"] == whole["P"] and second["Lz"] == whole["Lz"]
+
+
+def test_checkpoint_path_without_suffix_and_mismatch(tmp_path):
+    """a --checkpoint path without the .npz suffix used to restart from t = 0 on resume (np.savez appends the
+    suffix, the resume check looked for the bare name); a checkpoint of another run is now a clear error."""
+    import os
+    from paper_1803_01190_b200 import conservation
+    whole = conservation.run(10, 20, 5e-4, 10, "f64", verbose=False)
+    ck = str(tmp_path / "state")                         # no suffix
+    first = conservation.run(10, 20, 5e-4, 10, "f64", verbose=False, checkpoint=ck, stop_after=10)
+    assert first["steps"] == 10 and os.path.exists(ck + ".npz") and not os.path.exists(ck + ".tmp.npz")
+    second = conservation.run(10, 20, 5e-4, 10, "f64", verbose=False, checkpoint=ck)
+    assert second["steps"] == 20 and second["E"] == whole["E"] and second["times"] == whole["times"]
+    with pytest.raises(ValueError, match="one checkpoint file per run"):
+        conservation.run(10, 20, 5e-4, 10, "f32", verbose=False, checkpoint=ck)
