@@ -126,6 +126,9 @@ def test_bad_arguments_and_no_device(ppgrav):
     lib = ppgrav.lib()
     out = (ctypes.c_int64 * 16)()
     assert lib.pp_plan_query(0, 0, 0, out) == -1
+    assert lib.pp_plan_query(2 ** 28 + 1, 0, 0, out) == -1          # beyond the maximum size (2^28 bodies)
+    assert b"2^28" in lib.pp_last_error()
+    assert lib.pp_plan_query(2 ** 28, 1, 1, out) == 0 and out[0] * out[11] >= 2 ** 28     # the maximum size plans
     assert lib.pp_plan_query(10, 2, 0, out) == 0          # PP_MIXED plans like PP_F32
     assert lib.pp_plan_query(10, 3, 0, out) == -1
     assert b"precision" in lib.pp_last_error()
