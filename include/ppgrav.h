@@ -141,7 +141,7 @@ int pp_kick_drift(void* pos, void* vel, const void* acc, int64_t n, double kick,
  * nsteps == 0 only (re)computes acc.  Force evaluations performed: nsteps (+1 without PP_ACC_VALID).
  * Kernel launches: 1 (tile masses) + 3 for a cold start + 1 (kick+drift+pack) + 2 per interior step boundary
  * (pair sweep, fused update pass) + 2 (last sweep, finalize+kick) = 2 nsteps + 2 (+3); the symmetric sweep adds one per
- * call (block masses) and, beyond N = 2^21, one sweep and one fold launch per band of partner offsets.  For N <= 65536 the interior
+ * call (block masses) and, beyond N = 2^21, one sweep and two fold launches per band of partner offsets.  For N <= 65536 the interior
  * steps are replayed from a CUDA graph that is kept while the arguments do not change (also when `stream` is the legacy
  * default stream: the replay then runs on an internal stream, ordered with `stream` by events). */
 int pp_step_kdk(void* pos, void* vel, const void* mass, void* acc, void* pot, int64_t N, double dt, int64_t nsteps,
@@ -202,7 +202,8 @@ int pp_invariants_host(const void* pos, const void* vel, const void* mass, const
  *     PP_CFG_SYMMETRIC), [9] threads per CTA, [10] i-bodies per thread, [11] i-blocks,
  *     [12] ordered pairs (pair interactions) one evaluation serves: 1, or 2 for the symmetric sweep,
  *     [13] symmetric sweep: partner blocks H per block, [14] symmetric sweep: bands the partner blocks are cut into
- *     (1 = all j-side rows are kept at once), [15] reserved }. */
+ *     (1 = all j-side rows are kept at once), [15] bytes of device workspace the solve keeps (packed bodies, partial
+ *     sums, j-side rows; at most ~64 GB at any N: the rows are capped at 48 GB, 16 GB per band in a banded solve) }. */
 int pp_plan_query(int64_t N, int precision, int with_pot, int64_t* out16);
 
 /* How many j-tiles of a gravity solve of these masses have a common mass (and therefore run the pair loop without

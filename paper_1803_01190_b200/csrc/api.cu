@@ -195,7 +195,7 @@ struct JSide {
 };
 JSide jside(const Plan& p, const void* partial_j, const void* acc_j) {
     if (!p.sym) return {nullptr, 0, p.split};
-    if (p.sym_bands > 1) return {acc_j, 2, p.split * p.sym_bands};   // running TwoSum (value, error) of the bands
+    if (p.sym_bands > 1) return {acc_j, 2, 0};   // everything is already in the running TwoSum (value, error) sums
     return {partial_j, p.sym_h, p.split};
 }
 
@@ -343,9 +343,8 @@ int prepare_solve(Workspace* w, int64_t N, int precision, const void* mass, bool
     }
     s->n_pad = std::max(s->force.n_pad, s->force_pot.n_pad);
     const size_t body = 4 * sweep_elem_bytes(precision);
-    const size_t bands = sym ? (size_t)first.sym_bands : 1;   // a banded symmetric sweep keeps S partials per band
-    const size_t part = bands * std::max((size_t)s->force.split * (size_t)s->force.part_stride,
-                                         (size_t)s->force_pot.split * (size_t)s->force_pot.part_stride);
+    const size_t part = std::max((size_t)s->force.split * (size_t)s->force.part_stride,
+                                 (size_t)s->force_pot.split * (size_t)s->force_pot.part_stride);
     PP_TRY(ensure(w, B_PACKED, (size_t)s->n_pad * body, &s->packed));
     PP_TRY(ensure(w, B_PARTIAL, part * body, &s->partial));
     if (mass) PP_TRY(tile_masses(w, first, precision, mass, N, (int)g_cfg_equal_mass.load(), &s->tm, st));
@@ -517,7 +516,16 @@ int pp_plan_query(int64_t N, int precision, int with_pot, int64_t* out16) {
     out16[12] = p.sym ? 2 : 1;
     out16[13] = p.sym ? p.sym_h : 0;
     out16[14] = p.sym ? p.sym_bands : 0;
-    out16[15] = 0;
+    // bytes of workspace this solve keeps on the device: packed bodies, split-j partials, tile (and block) masses and,
+    // for the symmetric sweep, the j-side rows of one band plus the running sums of a banded solve
+    const size_t body = precision == PP_F64 ? 32 : 16;
+    size_t bytes = (size_t)p.n_pad * body + (size_t)p.split * (size_t)p.part_stride * body + (size_t)p.n_tiles * (body / 4);
+    if (p.sym) {
+        const size_t row_bytes = (size_t)p.part_stride * body;
+        bytes += (size_t)std::min(p.sym_rows, std::max(p.sym_h, 1)) * row_bytes + (size_t)p.n_iblocks * (body / 4);
+        if (p.sym_bands > 1) bytes += 2 * row_bytes;
+    }
+    out16[15] = (int64_t)bytes;
     return PP_OK;
 }
 

@@ -246,16 +246,19 @@ int launch_mg(const Plan& p, const double* packed, const double* tile_mass, cons
     auto kern = force_sym_f64_kernel<K.threads, K.ipt, K.tile_j, K.stages, MODE, GUARD>;
     PP_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));   // > 48 KB: opt-in
     dim3 grid(p.n_iblocks, p.split);
-    // bands of partner offsets (one band unless the j-side rows exceed the workspace cap): band b writes its i-side
-    // partials behind those of band b-1 and reuses the j-side rows, which fold_rows (update.cu) adds up in between
+    // bands of partner offsets (one band unless the j-side rows exceed the workspace cap): every band reuses BOTH the
+    // i-side partials and the j-side rows; in between, fold_rows (update.cu) adds them -- the S i-side partials first,
+    // then the band's rows, all in fixed order -- into the running TwoSum sums acc_j that finalize reads at the end
     for (int b = 0; b < p.sym_bands; ++b) {
         const int d0 = b * p.sym_rows, rows = std::min(p.sym_rows, p.sym_h - d0);
-        kern<<<grid, K.threads, smem, st>>>(packed, tile_mass, block_mass,
-                                            partial + (size_t)b * p.split * p.part_stride, partial_j, p.n_iblocks, d0,
-                                            rows, b == 0, p.part_stride, p.part_stride, eps2);
+        kern<<<grid, K.threads, smem, st>>>(packed, tile_mass, block_mass, partial, partial_j, p.n_iblocks, d0, rows,
+                                            b == 0, p.part_stride, p.part_stride, eps2);
         count_launch();
         PP_CUDA(cudaGetLastError());
-        if (p.sym_bands > 1) PP_TRY_RC(launch_fold_rows(partial_j, rows, p.part_stride, acc_j, b == 0, st));
+        if (p.sym_bands > 1) {
+            PP_TRY_RC(launch_fold_rows(partial, p.split, p.part_stride, acc_j, b == 0, st));
+            PP_TRY_RC(launch_fold_rows(partial_j, rows, p.part_stride, acc_j, false, st));
+        }
     }
     return PP_OK;
 }

@@ -145,7 +145,7 @@ Plan make_sym_plan(int64_t N, int precision, int mode, int sm_count, int64_t for
     const size_t row_bytes = (size_t)p.part_stride * elem;
     p.sym_rows = (int)std::max<size_t>(1, std::min<size_t>((size_t)std::max(p.sym_h, 1), rows_cap_bytes / row_bytes));
     p.sym_bands = std::max(1, (p.sym_h + p.sym_rows - 1) / p.sym_rows);
-    // every band keeps its own S i-side partials: a banded solve (N > 2^21: thousands of blocks) needs no split-j
+    // a banded solve (N > 2^21: thousands of blocks per band) needs no split-j
     if (p.sym_bands > 1 && forced_split < 1) p.split = 1;
     if (jbytes) *jbytes = std::max<size_t>((size_t)std::min(p.sym_rows, std::max(p.sym_h, 1)) * row_bytes, 16);
     if (abytes) *abytes = p.sym_bands > 1 ? 2 * row_bytes : 0;

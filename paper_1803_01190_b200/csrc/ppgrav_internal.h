@@ -219,7 +219,8 @@ int launch_force_f32(const Plan& p, const float* packed, const float* tile_mass,
                      double delta, int mode, cudaStream_t st);
 // symmetric sweep: i-side sums to partial[S][part_stride], j-side sums to partial_j[sym_h][part_stride] (same sign
 // convention, ready to be added); block_mass[I] = common mass of i-block I or NaN (launch_tile_mass_* with tile = block)
-// With p.sym_bands > 1 the rows are reused band after band and summed into acc_j[2][part_stride] (TwoSum value / error).
+// With p.sym_bands > 1 the partials and the rows are reused band after band and summed into acc_j[2][part_stride]
+// (TwoSum value / error), which is then all that finalize reads (split = 0, two j-side "rows").
 int launch_force_sym_f32(const Plan& p, const float* packed, const float* tile_mass, const float* block_mass,
                          float4* partial, float4* partial_j, float4* acc_j, double delta, int mode, cudaStream_t st);
 int launch_fold_rows(const float4* rows, int nrows, int64_t stride, float4* acc_j, bool first, cudaStream_t st);

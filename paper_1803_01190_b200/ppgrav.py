@@ -127,7 +127,7 @@ def pp_plan_query(N, precision, with_pot=False):
     _check(lib().pp_plan_query(int(N), int(precision), int(bool(with_pot)), out), "pp_plan_query")
     keys = ("i_per_cta", "tile_j", "split", "ctas", "ctas_per_sm", "sm_count", "pipe_ops_per_evaluation",
             "mufu_per_evaluation", "shape", "threads", "ipt", "i_blocks", "pairs_per_evaluation", "sym_partner_blocks",
-            "sym_bands")
+            "sym_bands", "workspace_bytes")
     d = dict(zip(keys, (int(v) for v in out)))
     # per ordered pair (pair interaction): what the roofline counts; one less on equal-mass tiles
     d["pipe_ops_per_pair"] = d["pipe_ops_per_evaluation"] / d["pairs_per_evaluation"]

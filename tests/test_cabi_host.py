@@ -129,6 +129,12 @@ def test_bad_arguments_and_no_device(ppgrav):
     assert lib.pp_plan_query(2 ** 28 + 1, 0, 0, out) == -1          # beyond the maximum size (2^28 bodies)
     assert b"2^28" in lib.pp_last_error()
     assert lib.pp_plan_query(2 ** 28, 1, 1, out) == 0 and out[0] * out[11] >= 2 ** 28     # the maximum size plans
+    # ... and its workspace fits the GPU: the banded symmetric sweep reuses its rows AND its partial sums, so the
+    # demand does not grow with the number of bands (round 2 first kept one set of partials per band: 137 GB at 2^25)
+    for n, cap in ((2 ** 20, 12), (2 ** 21, 40), (2 ** 23, 20), (2 ** 25, 24), (2 ** 28, 64)):
+        for prec in (0, 1):
+            q = ppgrav.pp_plan_query(n, prec, True)
+            assert q["shape"] == 3 and q["workspace_bytes"] <= cap << 30, (n, prec, q["workspace_bytes"] / 2 ** 30)
     assert lib.pp_plan_query(10, 2, 0, out) == 0          # PP_MIXED plans like PP_F32
     assert lib.pp_plan_query(10, 3, 0, out) == -1
     assert b"precision" in lib.pp_last_error()
